@@ -1,0 +1,461 @@
+"""Pins for the CPU oracle (oracle/sph_oracle.c) against what the paper and the mathematics fix.
+
+Each test names the pin (P1..P15) and the passage of PAPER.md it checks.
+None of these call the CUDA library.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+import oracle
+from paper_2104_00537_b200 import workloads as wl
+
+DP = 0.02
+H3 = 1.2 * math.sqrt(3) * DP
+H2 = 1.2 * math.sqrt(2) * DP
+
+
+def base_params(dim=3, **kw):
+    p = wl._params(dim, DP, 1.2, 10 * math.sqrt(9.81 * 0.3), (0, 0, -9.81), (0, 0, 0),
+                   (1, 1 if dim == 3 else 0, 1))
+    p.update(kw)
+    return p
+
+
+def periodic_lattice(n_side, dim=3, cell_div=1, g=(0, 0, 0)):
+    c = wl.periodic_cloud("lat", n_side, DP, 0.0, 5, cell_div=cell_div, dim=dim,
+                          vel_sigma=0.0, rho_sigma=0.0)
+    c.params["g"] = tuple(g)
+    return c
+
+
+# ---- P1: Wendland normalisation (Eq. 3 + Eq. 11) ------------------------
+def test_p1_wendland_integrates_to_one():
+    v3, _ = integrate.quad(lambda r: oracle.W(3, H3, r) * 4 * math.pi * r * r, 0, 2 * H3)
+    v2, _ = integrate.quad(lambda r: oracle.W(2, H2, r) * 2 * math.pi * r, 0, 2 * H2)
+    assert abs(v3 - 1) < 1e-10 and abs(v2 - 1) < 1e-10
+    assert oracle.W(3, H3, 2 * H3) == 0.0 and oracle.W(3, H3, 2.5 * H3) == 0.0
+    assert oracle.W(3, H3, 0.0) == pytest.approx(21 / (16 * math.pi * H3 ** 3), rel=1e-14)
+    assert oracle.W(2, H2, 0.0) == pytest.approx(7 / (4 * math.pi * H2 ** 2), rel=1e-14)
+
+
+def test_p1_lattice_partition_of_unity():
+    # sum_b W V over a cubic lattice incl. self = 1.00049 at h = 1.2 sqrt(3) dp
+    r = np.arange(-5, 6)
+    X, Y, Z = np.meshgrid(r, r, r, indexing="ij")
+    d = np.sqrt(X ** 2 + Y ** 2 + Z ** 2).ravel() * DP
+    s = sum(oracle.W(3, H3, float(x)) for x in d) * DP ** 3
+    assert abs(s - 1.00049) < 2e-5
+
+
+# ---- P2: kernel gradient (derived from Eq. 11) -------------------------------------------------
+@pytest.mark.parametrize("dim,h", [(3, H3), (2, H2)])
+def test_p2_gradient_matches_finite_difference(dim, h):
+    for q in (0.05, 0.3, 0.7216878, 1.0, 1.5, 1.95):
+        r = q * h
+        e = 1e-6 * h
+        fd = (oracle.W(dim, h, r + e) - oracle.W(dim, h, r - e)) / (2 * e)  # dW/dr
+        assert oracle.fab(dim, h, r) * r == pytest.approx(fd, rel=2e-8, abs=1e-6)
+    assert oracle.fab(dim, h, 2 * h) == 0.0
+    assert oracle.fab(dim, h, 0.0) < 0  # finite at r = 0: grad W = f * r_ab = 0 there (A17)
+
+
+# ---- P3: Tait EOS (Eq. 28) ---------------------------------------------------
+def test_p3_eos():
+    p = base_params()
+    assert oracle.eos(p, p["rho0"]) == 0.0
+    e = 1e-4
+    dP = (oracle.eos(p, p["rho0"] + e) - oracle.eos(p, p["rho0"] - e)) / (2 * e)
+    assert dP == pytest.approx(p["c0"] ** 2, rel=1e-8)   # c_s = sqrt(dP/drho) at rho0
+    # 1 % density variation -> P = B(1.01^7 - 1)
+    B = p["c0"] ** 2 * 1000 / 7
+    assert oracle.eos(p, 1010.0) == pytest.approx(B * (1.01 ** 7 - 1), rel=1e-12)
+
+
+# ---- P4: neighbour search: brute force == cell list; lattice counts -----------------------------
+@pytest.mark.parametrize("cell_div", [1, 2])
+def test_p4_bruteforce_equals_celllist_config0(cell_div):
+    c = wl.config(0, cell_div=cell_div)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    a = st.interactions(mode=0)
+    b = st.interactions(mode=1)
+    assert np.array_equal(a["nbcount"], b["nbcount"])
+    assert int(a["nbcount"].sum()) == 1738918          # SURVEY 8(d), config 0 lattice count
+    F = c.ptype == 0
+    assert int(a["nbcount"][~F].sum()) == 225331       # B<-F
+    assert int(a["nbcount"][F].sum()) == 1288256 + 225331
+
+
+@pytest.mark.parametrize("dim,periodic,cell_div", [(3, (0, 0, 0), 1), (3, (1, 1, 1), 1),
+                                                   (3, (1, 1, 1), 2), (2, (0, 0, 0), 1),
+                                                   (2, (1, 0, 1), 2), (3, (0, 0, 0), 2)])
+def test_p4_bruteforce_equals_celllist_random(dim, periodic, cell_div):
+    box = (0.6, 0.6 if dim == 3 else 0.0, 0.6)
+    n = 3000 if dim == 3 else 1200
+    c = wl.random_cloud("rc", n, box, DP, 99 + dim + cell_div, dim=dim, periodic=periodic,
+                        cell_div=cell_div)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    a = st.interactions(mode=0)
+    b = st.interactions(mode=1)
+    assert np.array_equal(a["nbcount"], b["nbcount"])
+    assert a["nbcount"].sum() > 10 * n
+    # same neighbour sets, but the two modes visit them in different orders -> rounding only
+    np.testing.assert_allclose(a["acc"], b["acc"], rtol=1e-9, atol=1e-9 * np.abs(a["acc"]).max())
+    np.testing.assert_allclose(a["drho"], b["drho"], rtol=1e-9, atol=1e-9 * np.abs(a["drho"]).max())
+    assert a["viscmax"] == b["viscmax"]
+
+
+def test_p4_neighbour_count_independent_of_numpy_bruteforce():
+    # independent numpy enumeration in double on an irregular cloud; counts must agree except for
+    # pairs within rounding of the cut-off (reported by the oracle as n_diff)
+    c = wl.random_cloud("rc", 1500, (0.5, 0.5, 0.5), DP, 4242)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    r = st.interactions(mode=0)
+    x = st.pos
+    d2 = ((x[:, None, :] - x[None, :, :]) ** 2).sum(-1)
+    within = d2 < (2 * c.params["h"]) ** 2
+    np.fill_diagonal(within, False)
+    bb = (c.ptype[:, None] != 0) & (c.ptype[None, :] != 0)
+    cnt = (within & ~bb).sum(1)
+    assert np.abs(cnt.astype(np.int64) - r["nbcount"].astype(np.int64)).sum() <= r["n_diff"] + 2
+    assert r["n_diff"] <= 4
+
+
+@pytest.mark.parametrize("dim,n_side,expect,cell_div", [(3, 21, 304, 1), (3, 21, 304, 2),
+                                                        (2, 34, 36, 1), (2, 34, 36, 2)])
+def test_p4_lattice_neighbour_counts(dim, n_side, expect, cell_div):
+    # h = 1.2 sqrt(d) dp: 304 (3-D), 36 (2-D) neighbours on an unjittered lattice (
+    # paper: "typically 40 in 2D and around 250 in 3D")
+    c = periodic_lattice(n_side, dim=dim, cell_div=cell_div)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    r = st.interactions(mode=1)
+    assert (r["nbcount"] == expect).all()
+
+
+def test_p4_count_250_when_2h_is_4dp():
+    # "more than 268 neighbouring particles in 3-D (when 2h is ... four times the initial
+    # interparticle distance)" PAPER.md:597: continuum 268.1; strict (<) lattice count is 250.
+    c = periodic_lattice(24, dim=3)
+    c.params["h"] = 2.0 * DP
+    L = 24 * DP
+    c.params["cell_size"] = L / math.floor(L / (4 * DP))
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    r = st.interactions(mode=1)
+    assert (r["nbcount"] == 250).all()
+
+
+# ---- P5/P6: antisymmetry -> momentum and diffusion conservation ------------------
+def test_p5_p6_conservation_periodic_cloud():
+    c = wl.periodic_cloud("pc", 16, DP, 0.2, 7, rho_sigma=0.005)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    r = st.interactions()
+    m = 1000.0 * DP ** 3
+    tot = (m * r["acc"]).sum(0)
+    scale = np.abs(m * r["acc"]).sum(0).max()
+    assert np.abs(tot).max() < 1e-11 * scale             # sum m F = 0 (g = 0, no boundaries)
+    p0 = dict(c.params, delta=0.0)
+    r0 = oracle.interactions(p0, st.cell, st.u, st.out, st.vel, st.rho, st.ptype)
+    D = r["drho"] - r0["drho"]
+    assert np.abs(D).max() > 1e-3
+    VD = (m / st.rho) * D
+    assert abs(VD.sum()) < 1e-10 * np.abs(VD).sum()      # sum V_a D_a = 0
+    # gravity only shifts F by g
+    pg = dict(c.params, g=(0.0, 0.0, -9.81))
+    rg = oracle.interactions(pg, st.cell, st.u, st.out, st.vel, st.rho, st.ptype)
+    np.testing.assert_allclose(rg["acc"] - r["acc"], np.tile([0, 0, -9.81], (c.n, 1)), atol=1e-9)
+
+
+# ---- P7: diffusion sign and magnitude (Eq. 17-18, reading A3) -----------------------------------
+def test_p7_diffusion_is_diffusive():
+    # rho = rho0 + A x^2 on a full-support lattice: D_a -> delta h c0 * laplacian(rho) = delta h c0 2A
+    n = 17
+    c = wl.dam_break("blk", 3, DP, (n, n, n), (n, n, n), 0.0, 1, 0.3)
+    keep = c.ptype == 0
+    pos = c.pos[keep]
+    A = 200.0
+    x0 = pos[:, 0].mean()
+    rho = 1000.0 + A * (pos[:, 0] - x0) ** 2
+    p = dict(c.params, g=(0, 0, 0))
+    st = oracle.State(p, pos, np.zeros_like(pos), rho, np.zeros(len(pos), np.uint8))
+    r1 = st.interactions()
+    st0 = oracle.State(dict(p, delta=0.0), pos, np.zeros_like(pos), rho, np.zeros(len(pos), np.uint8))
+    r0 = st0.interactions()
+    D = r1["drho"] - r0["drho"]
+    centre = np.argmin(((pos - pos.mean(0)) ** 2).sum(1))
+    assert r1["nbcount"][centre] == 304
+    expect = p["delta"] * p["h"] * p["c0"] * 2 * A
+    assert D[centre] == pytest.approx(expect, rel=0.03)
+    # a particle whose neighbours are all denser gains density
+    rho2 = np.full(len(pos), 1001.0); rho2[centre] = 1000.0
+    st2 = oracle.State(p, pos, np.zeros_like(pos), rho2, np.zeros(len(pos), np.uint8))
+    assert st2.interactions()["drho"][centre] > 0
+
+
+# ---- P8: continuity against Eq. 12 (drho/dt = -rho div v) ---------------------------------------
+def test_p8_continuity_linear_velocity_field():
+    n = 15
+    c = wl.dam_break("blk", 3, DP, (n, n, n), (n, n, n), 0.0, 1, 0.3)
+    keep = c.ptype == 0
+    pos = c.pos[keep]
+    G = np.array([[0.7, 0.2, -0.1], [0.05, -0.3, 0.4], [0.3, -0.6, 0.25]])
+    vel = (pos - pos.mean(0)) @ G.T
+    p = dict(c.params, g=(0, 0, 0), delta=0.0)
+    st = oracle.State(p, pos, vel.astype(np.float32), np.full(len(pos), 1000.0), np.zeros(len(pos), np.uint8))
+    r = st.interactions()
+    centre = np.argmin(((pos - pos.mean(0)) ** 2).sum(1))
+    # lattice moment sum_b V_b f_ab r_i r_j = -1.00036 delta_ij at h = 1.2 sqrt(3) dp
+    assert r["drho"][centre] == pytest.approx(-1000.0 * np.trace(G) * 1.00036, rel=2e-4)
+    # uniform translation adds nothing
+    st.vel += np.array([3.0, -2.0, 1.0])
+    r2 = st.interactions()
+    assert r2["drho"][centre] == pytest.approx(r["drho"][centre], rel=1e-9)
+
+
+# ---- P9: uniform state -----------------------------------------------------------------------------
+@pytest.mark.parametrize("dim,n_side", [(3, 24), (2, 32)])
+def test_p9_uniform_lattice_feels_only_gravity(dim, n_side):
+    c = periodic_lattice(n_side, dim=dim, g=(0, 0, -9.81))
+    # cells of 8 dp: lattice offsets (i + 1/2)/8 are dyadic, so the canonical 2^-22 grid (C1) holds the
+    # lattice exactly and the symmetric cancellation is exact up to rounding of the sums
+    c.params["cell_size"] = 8 * DP
+    rho = np.full(c.n, 1003.0)  # P != 0 but uniform: sum grad W = 0 by symmetry
+    st = oracle.State(c.params, c.pos, c.vel, rho, c.ptype)
+    r = st.interactions()
+    B = c.params["c0"] ** 2 * 1000 / 7
+    pair_scale = 2 * B * (1.003 ** 7 - 1) / 1003.0 ** 2 * 1000 * DP ** dim * abs(oracle.fab(dim, c.params["h"], DP)) * DP
+    np.testing.assert_allclose(r["acc"], np.tile([0, 0, -9.81], (c.n, 1)), atol=1e-9 * pair_scale * 300 + 1e-12)
+    assert np.abs(r["drho"]).max() < 1e-9
+    assert r["viscmax"] == 0.0
+
+
+# ---- P10 / P11: two particles ------------------------------------------------------------------------
+def two_particles(va, rho_b=1010.0, alpha=0.01, delta=0.1):
+    p = base_params(g=(0.0, 0.0, 0.0), alpha=alpha, delta=delta)
+    p["domain_min"] = (-0.2, -0.2, -0.2)
+    p["domain_max"] = (0.2, 0.2, 0.2)
+    # positions chosen so the canonical state (C1) reproduces them to ~1e-9
+    pos = np.array([[0.0, 0.0, 0.0], [0.03, 0.0, 0.0]])
+    vel = np.array([va, [0.0, 0.0, 0.0]], np.float32)
+    rho = np.array([1000.0, rho_b])
+    st = oracle.State(p, pos, vel, rho, np.zeros(2, np.uint8))
+    return p, st
+
+
+def test_p11_worked_two_particle_example(golden):
+    g = golden("two_particle.txt")
+    p, st = two_particles([0.5, 0.0, 0.0])
+    assert p["h"] == pytest.approx(g["h"], rel=1e-13)
+    assert p["c0"] == pytest.approx(g["c0"], rel=1e-13)
+    assert oracle.alphaD(3, p["h"]) == pytest.approx(g["alphaD"], rel=1e-12)
+    r_ab = float(np.linalg.norm(st.pos[0] - st.pos[1]))
+    assert r_ab == pytest.approx(0.03, abs=3e-8)            # canonical quantisation (C1)
+    tol = dict(rel=2e-5)                                    # 2^-22 grid moves r by <= ~1e-6 relative
+    assert oracle.W(3, p["h"], 0.03) == pytest.approx(g["W"], rel=1e-12)
+    assert oracle.fab(3, p["h"], 0.03) == pytest.approx(g["f_ab"], rel=1e-12)
+    assert oracle.fab(3, p["h"], 0.03) * (-0.03) == pytest.approx(g["gradW_x"], rel=1e-12)
+    assert oracle.eos(p, 1010.0) == pytest.approx(g["P_b"], rel=1e-12)
+    r = st.interactions(mode=0)
+    assert list(r["nbcount"]) == [1, 1]
+    assert r["viscmax"] == pytest.approx(abs(g["mu_ab"]), **tol)
+    assert r["drho"][0] == pytest.approx(g["R_a_cont"] + g["D_a"], **tol)
+    assert r["drho"][1] == pytest.approx(g["R_b_cont"] + g["D_b"], **tol)
+    assert r["acc"][0, 0] == pytest.approx(g["F_a_x"], **tol)
+    assert r["acc"][1, 0] == pytest.approx(g["F_b_x"], **tol)
+    assert abs(r["acc"][0, 0] + r["acc"][1, 0]) < 1e-12
+    # continuity and diffusion separately (delta = 0 run)
+    p0, st0 = two_particles([0.5, 0.0, 0.0], delta=0.0)
+    r0 = st0.interactions(mode=0)
+    assert r0["drho"][0] == pytest.approx(g["R_a_cont"], **tol)
+    assert r["drho"][0] - r0["drho"][0] == pytest.approx(g["D_a"], **tol)
+    assert r["drho"][1] - r0["drho"][1] == pytest.approx(g["D_b"], **tol)
+    # viscosity separately (alpha = 0 run): Pi_ab enters F as -m Pi f r_ab
+    pa, sta = two_particles([0.5, 0.0, 0.0], alpha=0.0)
+    ra = sta.interactions(mode=0)
+    dF = r["acc"][0, 0] - ra["acc"][0, 0]
+    assert dF == pytest.approx(-g["m"] * g["Pi_ab"] * g["f_ab"] * (-0.03), **tol)
+
+
+def test_p10_viscosity_only_for_approaching_pairs():
+    _, app = two_particles([0.5, 0.0, 0.0])        # a moves towards b: v_ab.r_ab < 0
+    _, app0 = two_particles([0.5, 0.0, 0.0], alpha=0.0)
+    _, sep = two_particles([-0.5, 0.0, 0.0])       # separating
+    _, sep0 = two_particles([-0.5, 0.0, 0.0], alpha=0.0)
+    d_app = app.interactions(0)["acc"] - app0.interactions(0)["acc"]
+    d_sep = sep.interactions(0)["acc"] - sep0.interactions(0)["acc"]
+    assert np.all(d_sep == 0.0)                    # Pi_ab = 0 for v_ab.r_ab >= 0 (Eq. 21)
+    assert d_app[0, 0] < 0 and d_app[1, 0] > 0     # Pi > 0: extra repulsion (a pushed to -x)
+    assert d_app[0, 0] == pytest.approx(-d_app[1, 0], rel=1e-12)   # symmetric in a <-> b
+    # tangential relative motion: v_ab.r_ab = 0 -> no viscosity, no continuity
+    _, tan = two_particles([0.0, 0.5, 0.0], rho_b=1000.0)
+    rt = tan.interactions(0)
+    assert rt["viscmax"] == 0.0 and np.all(rt["drho"] == 0.0)
+
+
+def test_boundary_pairs_eq36():
+    # DBC (Eq. 36): boundary a: continuity over fluid b only, no momentum, no D_a;
+    # B<-B pairs never evaluated.
+    p = base_params(g=(0.0, 0.0, -9.81))
+    p["domain_min"] = (-0.2, -0.2, -0.2); p["domain_max"] = (0.2, 0.2, 0.2)
+    pos = np.array([[0.0, 0, 0], [0.03, 0, 0], [0.0, 0.03, 0]])
+    vel = np.array([[0.0, 0, 0], [-0.4, 0, 0], [0, 0, 0]], np.float32)
+    rho = np.array([1002.0, 1001.0, 1003.0])
+    typ = np.array([1, 0, 1], np.uint8)              # B, F, B
+    st = oracle.State(p, pos, vel, rho, typ)
+    r = st.interactions(0)
+    assert list(r["nbcount"]) == [1, 2, 1]           # B0<-F1 ; F1<-B0,B2 ; B2<-F1 (B0-B2 in range but skipped)
+    assert np.all(r["acc"][0] == 0) and np.all(r["acc"][2] == 0)
+    m = 1000 * DP ** 3
+    f = oracle.fab(3, p["h"], float(np.linalg.norm(st.pos[0] - st.pos[1])))
+    rab = st.pos[0] - st.pos[1]
+    vab = st.vel[0] - st.vel[1]
+    assert r["drho"][0] == pytest.approx(1002.0 * m / 1001.0 * float(vab @ rab) * f, rel=1e-12)
+    # fluid particle: no diffusion from boundary neighbours by default (A4) ...
+    r_nod = oracle.interactions(dict(p, delta=0.0), st.cell, st.u, st.out, st.vel, st.rho, typ, 0)
+    assert r["drho"][1] == r_nod["drho"][1]
+    # ... but with ddt_over_boundary = 1 it does
+    r_ddt = oracle.interactions(dict(p, ddt_over_boundary=1), st.cell, st.u, st.out, st.vel, st.rho, typ, 0)
+    assert r_ddt["drho"][1] != r["drho"][1]
+    assert r["acc"][1, 2] == pytest.approx(-9.81, abs=1e-9)   # pressure forces are in-plane here
+
+
+# ---- P12: dt (Eq. 35) ------------------------------------------------------------
+def test_p12_dt_closed_form():
+    c = wl.config(0)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    r = st.interactions()
+    dt = oracle.dt(c.params, r["acc"], c.ptype, st.out, r["viscmax"])
+    h, c0 = c.params["h"], c.params["c0"]
+    assert math.sqrt(h / 9.81) == pytest.approx(0.0650956, rel=1e-5)
+    assert h / c0 == pytest.approx(0.00242313, rel=1e-5)
+    assert dt == pytest.approx(0.2 * min(math.sqrt(h / 9.81), h / c0), rel=1e-12)
+    assert dt == pytest.approx(4.84626e-4, rel=1e-5)
+    # force-limited regime
+    acc = np.zeros((c.n, 3)); acc[np.argmax(c.ptype == 0), 0] = 1e4
+    assert oracle.dt(c.params, acc, c.ptype, st.out, 0.0) == pytest.approx(0.2 * math.sqrt(h / 1e4), rel=1e-12)
+    # a boundary particle's entry is ignored (fluid only, A13)
+    acc = np.zeros((c.n, 3)); acc[np.argmax(c.ptype != 0), 0] = 1e9
+    assert oracle.dt(c.params, acc, c.ptype, st.out, 0.0) == pytest.approx(0.2 * h / c0, rel=1e-12)
+    # viscous term
+    assert oracle.dt(c.params, np.zeros((c.n, 3)), c.ptype, st.out, 5.0) == pytest.approx(0.2 * h / (c0 + 5.0), rel=1e-12)
+
+
+# ---- P13: integrator (Eq. 33-34) ---------------------------------------------------
+def test_p13_free_fall_is_exact():
+    p = base_params(g=(0.0, 0.0, -9.81))
+    p["domain_min"] = (-1, -1, -1); p["domain_max"] = (1, 1, 1)
+    pos = np.array([[0.1, 0.2, 0.3]]); vel = np.array([[0.3, -0.1, 0.5]], np.float32)
+    st = oracle.State(p, pos, vel, np.array([1000.0]), np.zeros(1, np.uint8))
+    x0 = st.pos.copy(); v0 = st.vel.copy()
+    st.step(3)
+    t = st.t
+    dts = np.array(st.dt_hist)
+    assert np.allclose(dts, 0.2 * min(math.sqrt(p["h"] / 9.81), p["h"] / p["c0"]), rtol=1e-12)
+    g = np.array([0, 0, -9.81])
+    np.testing.assert_allclose(st.vel[0], v0[0] + g * t, rtol=1e-12)
+    q = 2 ** -22 * oracle.grid(p)[0]
+    np.testing.assert_allclose(st.pos[0], x0[0] + v0[0] * t + 0.5 * g * t * t, atol=6 * q)  # 2 re-quantisations/step
+    assert st.rho[0] == 1000.0
+
+
+def test_p13_density_pade_form_two_particles():
+    # Eq. 34: rho^{n+1} = rho^n (2 - eps)/(2 + eps), eps = -(R^{n+1/2}/rho^{n+1/2}) dt.
+    # Checked from quantities of an independent second State advanced by hand to n+1/2.
+    p, st = two_particles([0.5, 0.0, 0.0], rho_b=1000.0, alpha=0.0, delta=0.0)
+    r_n = st.interactions(0)
+    dt = oracle.dt(p, r_n["acc"], st.ptype, st.out, r_n["viscmax"])
+    x_n, v_n, rho_n = st.pos.copy(), st.vel.copy(), st.rho.copy()
+    half = oracle.State(p, x_n + 0.5 * dt * v_n, np.zeros((2, 3)), rho_n + 0.5 * dt * r_n["drho"], st.ptype)
+    half.vel = v_n + 0.5 * dt * r_n["acc"]
+    r_h = half.interactions(0)
+    eps = -(r_h["drho"] / half.rho) * dt
+    st.step(1)
+    assert st.dt_hist[0] == pytest.approx(dt, rel=1e-14)
+    np.testing.assert_allclose(st.rho, rho_n * (2 - eps) / (2 + eps), rtol=1e-13)
+    np.testing.assert_allclose(st.vel, v_n + dt * r_h["acc"], rtol=1e-12, atol=1e-15)
+    q = 2 ** -22 * oracle.grid(p)[0]
+    np.testing.assert_allclose(st.pos, x_n + dt * 0.5 * (st.vel + v_n), atol=2 * q)
+    assert np.all(st.rho > 1000.0)    # approaching particles compress
+
+
+def test_p13_second_order_convergence():
+    # the predictor-corrector is second order accurate in time: halving dt (via CFL)
+    # must cut the error of v by ~4x.  A dropped half step or a wrong state in the corrector gives 2x.
+    c = wl.periodic_cloud("pc", 8, DP, 0.15, 11, vel_sigma=0.02, rho_sigma=0.002)
+    T = None
+    sols = []
+    for k, cfl in enumerate((0.2, 0.1, 0.05, 0.0125)):
+        p = dict(c.params, cfl=cfl)
+        st = oracle.State(p, c.pos, c.vel, c.rho, c.ptype)
+        nsteps = 4 * (2 ** k) if k < 3 else 64
+        st.step(nsteps)
+        sols.append((st.t, st.vel.copy(), st.rho.copy()))
+    # variable dt makes end times differ slightly: compare at matched time by linear rescale of error
+    t0 = sols[0][0]
+    for t, _, _ in sols:
+        assert t == pytest.approx(t0, rel=2e-2)
+    ref_v, ref_r = sols[3][1], sols[3][2]
+    e = [np.abs(s[1] - ref_v).max() for s in sols[:3]]
+    assert e[0] > 0
+    # end-time mismatch pollutes the finest comparison; use the two coarse ratios loosely
+    assert e[0] / e[1] > 2.6
+
+
+def test_momentum_conserved_over_steps():
+    c = wl.periodic_cloud("pc", 10, DP, 0.2, 3, rho_sigma=0.003)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    p0 = st.vel.sum(0)
+    st.step(5)
+    p1 = st.vel.sum(0)
+    assert np.abs(p1 - p0).max() < 1e-10 * np.abs(st.vel).sum()
+    assert st.out.sum() == 0 and len(st.rho) == c.n        # P15: no particle lost
+
+
+# ---- P14: hydrostatic column (north_star) -----------------------------------------------------------
+def test_p14_hydrostatic_column_holds_pressure():
+    c = wl.hydrostatic_column("col", DP, (8, 8, 14), 10)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    st.step(120)
+    F = c.ptype == 0
+    p = c.params
+    assert np.abs(st.vel[F]).max() < p["c0"] / 10
+    depth = 10 * DP - st.pos[F, 2]
+    P = np.array([oracle.eos(p, float(r)) for r in st.rho[F]])
+    deep = depth > 0.1
+    ratio = P[deep] / (1000 * 9.81 * depth[deep])
+    assert 0.8 < np.median(ratio) < 1.2
+    assert st.out.sum() == 0
+
+
+# ---- C1: canonical positions ------------------------------------------------------------------------
+def test_c1_canonical_state_properties():
+    c = wl.random_cloud("rc", 5000, (0.5, 0.5, 0.5), DP, 1)
+    cell, u, out = oracle.canonicalize(c.params, c.pos)
+    assert out.sum() == 0
+    assert (u >= 0).all() and (u < 1).all()
+    assert np.array_equal(u * 2 ** 22, np.round(u * 2 ** 22))          # on the 2^-22 grid
+    cs, nc, r2u = oracle.grid(c.params)
+    assert r2u == np.float32(1.0)
+    x = oracle.position(c.params, cell, u)
+    assert np.abs(x - c.pos).max() <= 0.5 * 2 ** -22 * cs * (1 + 1e-9)
+    cell2, u2, _ = oracle.canonicalize(c.params, x)                   # idempotent
+    assert np.array_equal(cell, cell2) and np.array_equal(u, u2)
+    # out-of-grid flag
+    bad = c.pos.copy(); bad[0, 0] = 10.0; bad[1, 2] = -5.0
+    _, _, o = oracle.canonicalize(c.params, bad)
+    assert o[0] == 1 and o[1] == 1 and o[2:].sum() == 0
+
+
+def test_c3_keys_sort_cellstart():
+    c = wl.dam_break("t", 3, DP, (12, 8, 8), (5, 8, 6), 0.01, 3, 0.3, shuffle=True)
+    cell, u, out = oracle.canonicalize(c.params, c.pos)
+    key, perm, cellstart = oracle.neighbour_list(c.params, cell, u, c.ptype, out)
+    cs, nc, _ = oracle.grid(c.params)
+    ncells = nc[0] * nc[1] * nc[2]
+    lin = cell[:, 0] + nc[0] * (cell[:, 1] + nc[1] * cell[:, 2])
+    assert np.array_equal(key, np.where(c.ptype == 0, ncells, 0) + lin)
+    assert np.array_equal(perm, np.argsort(key, kind="stable"))       # library stable sort as a step-check
+    sk = key[perm]
+    assert np.array_equal(cellstart, np.searchsorted(sk, np.arange(2 * ncells + 2), side="left"))
+    assert cellstart[ncells] == c.n_bound and cellstart[-1] == c.n
