@@ -1,0 +1,170 @@
+/*
+ * sph.h -- C ABI of libsph_b200.so: the neighbour-search + particle-interaction + system-update
+ * hot path of weakly compressible SPH (arxiv 2104.00537, DualSPHysics v5.0 paper) on one B200.
+ *
+ * Reference for every call: /root/reference/PAPER.md (cited as PAPER.md:<line>) and the readings
+ * A1..A20 / canonical definitions C1..C3 listed in DESIGN.md.
+ *
+ * General conventions
+ *   - Every function returns SPH_OK (0) or a negative SPH_E_* code; nothing throws or exits.
+ *     sph_last_error() gives a human-readable message for the last failure on that context.
+ *   - "host" pointers are plain CPU memory owned by the caller; the library copies and never
+ *     retains them.  All device state is owned by the library and released by sph_destroy().
+ *   - Device memory is obtained through params.dev_alloc / dev_free when given (PyTorch's caching
+ *     allocator in the Python binding), else cudaMalloc/cudaFree.  All work is enqueued on
+ *     params.cuda_stream (a cudaStream_t; NULL = legacy default stream).
+ *   - Calls are asynchronous on that stream except sph_load_particles (synchronous H2D from
+ *     pageable memory), sph_read_state, sph_get_info and sph_get_timings, which synchronise it.
+ *   - Asynchronous device-side faults (NaN in an acceleration, > 2^32-2 keys) set a device flag
+ *     that the next synchronising call reports as SPH_E_NAN / SPH_E_OVERFLOW.
+ *   - One context per host thread at a time.  There is no CPU fallback: without a CUDA device
+ *     sph_create fails with SPH_E_CUDA.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_OK 0
+#define SPH_E_BADARG (-1)   /* invalid parameter or NULL pointer                     */
+#define SPH_E_NOMEM (-2)    /* device allocation failed                              */
+#define SPH_E_CUDA (-3)     /* CUDA runtime error (message in sph_last_error)        */
+#define SPH_E_STATE (-4)    /* call out of order (e.g. step before load)             */
+#define SPH_E_OVERFLOW (-5) /* grid too large for 32-bit keys / buffer too small     */
+#define SPH_E_NAN (-6)      /* non-finite acceleration or density detected on device */
+
+typedef struct sph_ctx sph_ctx; /* opaque, owned by the library */
+
+typedef void* (*sph_alloc_fn)(size_t bytes, void* user); /* returns a device pointer or NULL */
+typedef void (*sph_free_fn)(void* dev_ptr, void* user);
+
+/* Parameters of the problem as the paper states it (dp, h: PAPER.md:60,78; rho0, c0, gamma:
+ * 214-218, Eq. 28; alpha: 176-178, Eq. 21; delta: 153, Eq. 17; g: 129; CFL: 285-288, Eq. 35). */
+typedef struct sph_params {
+  int32_t dim;               /* 2 or 3.  The 2-D plane is (x, z); y is ignored (A19).                */
+  double dp;                 /* initial particle spacing; particle mass m = rho0 * dp^dim (A9)       */
+  double h;                  /* smoothing length; support radius 2h (Eq. 4, 11)                      */
+  double rho0, c0, gamma;    /* Tait EOS, Eq. 28: P = c0^2 rho0/gamma ((rho/rho0)^gamma - 1)         */
+  double alpha;              /* artificial viscosity coefficient, Eq. 21                             */
+  double delta;              /* density diffusion coefficient, Eq. 17-18 (Molteni-Colagrossi)        */
+  double g[3];               /* external acceleration f of Eq. 22                                    */
+  double cfl;                /* C_CFL of Eq. 35                                                      */
+  double domain_min[3];      /* cell-grid extent; particles outside on a non-periodic axis are       */
+  double domain_max[3];      /*   flagged "out", excluded and counted (A16)                          */
+  int32_t periodic[3];       /* periodic axes; length must be a multiple of cell size */
+  double eta2_coef;          /* eta^2 = eta2_coef * h^2, paper value 0.001 (A6)                      */
+  int32_t ddt_over_boundary; /* 0: D_a sums fluid neighbours only (A4); 1: all neighbours            */
+  int32_t rho_bound_floor;   /* 1: clamp boundary density at rho0 (A10); default 0                   */
+  int32_t cell_div;          /* k in {1,2,3}: cubic cells of size 2h/k, (2k+1)^dim-cell stencil.     */
+                             /*   k=1: "cells of size 2h"; k=2: "size h" (635)        */
+  double cell_size;          /* 0 -> 2h/k; else >= 2h/k, one value for all axes (C1)                 */
+  int32_t pi_kernel;         /* interaction kernel: 0 auto, 1 gather (thread/particle), 2 tiled smem */
+  int32_t count_neighbours;  /* 1: keep per-particle neighbour counts (SPH_NBCOUNT); costs a store   */
+  sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
+  sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */
+  void* user;                /* passed back to dev_alloc / dev_free                                  */
+  void* cuda_stream;         /* cudaStream_t                                                         */
+} sph_params;
+
+/* Derived quantities and counters, filled by sph_get_info (synchronises the stream). */
+typedef struct sph_info {
+  int64_t n;               /* particles loaded                                                       */
+  int64_t n_out;           /* particles currently flagged out of the grid (A16)                      */
+  int64_t n_bound;         /* boundary particles in the grid (sorted first, C3)                      */
+  int32_t ncell[3];        /* cells per axis                                                         */
+  int64_t ncells;          /* ncell[0]*ncell[1]*ncell[2]; keys run 0 .. 2*ncells (C3)                */
+  double cell_size;        /* cs                                                                     */
+  float r2u;               /* (2h/cs)^2 as float: squared support in cell units (C2)                 */
+  uint64_t n_interactions; /* ordered neighbour pairs found by the last interaction pass             */
+  uint64_t n_interactions_total; /* accumulated over all passes since load                           */
+  int64_t steps_done;
+  double t, dt;            /* simulated time and last step's dt                                      */
+  int32_t pi_kernel;       /* kernel actually used                                                   */
+  int32_t device_flags;    /* bit 0: non-finite value seen; bit 1: key overflow                      */
+} sph_info;
+
+/* Accumulated device time per phase, measured with CUDA events on the context's stream while
+ * profiling is on (sph_set_profiling).  Phases follow SURVEY.md 8(a): a1 key, a2 sort,
+ * a3 cell-range table, a4 reorder (+a7 EOS), a5/a6 interaction, a8 dt, a9 update. */
+typedef struct sph_timings {
+  double ms_key, ms_sort, ms_cellstart, ms_reorder, ms_interaction, ms_dt, ms_update;
+  int64_t n_nl_builds, n_interaction_passes, n_kernel_launches;
+} sph_timings;
+
+/* What sph_read_state copies out.  Per-particle fields come back in the caller's ORIGINAL particle
+ * order; SPH_KEY / SPH_PERM / SPH_CELLSTART describe the sorted order of the last neighbour-list
+ * build (C3). */
+enum sph_field {
+  SPH_POS = 1,        /* double[n*3]  x = domain_min + (cell + u) * cs  (inverse of C1)             */
+  SPH_VEL = 2,        /* float[n*3]                                                                 */
+  SPH_RHO = 3,        /* float[n]                                                                   */
+  SPH_ACC = 4,        /* float[n*3]   dv/dt of the last pass incl. g (Eq. 22); 0 for boundary       */
+  SPH_DRHODT = 5,     /* float[n]     d rho/dt of the last pass (Eq. 15 / 36)                       */
+  SPH_KEY = 6,        /* uint32[n]    sorted keys                                                   */
+  SPH_PERM = 7,       /* uint32[n]    original index of the j-th sorted particle                    */
+  SPH_CELLSTART = 8,  /* uint32[2*ncells+2]  cellstart[k] = #{keys < k}                             */
+  SPH_NBCOUNT = 9,    /* uint32[n]    neighbours per particle (needs count_neighbours = 1)          */
+  SPH_CELL = 10,      /* int32[n*3]   canonical cell coordinates (C1)                               */
+  SPH_OFFSET = 11,    /* float[n*3]   canonical in-cell offsets u in [0,1) on the 2^-22 grid (C1)   */
+  SPH_PRESS = 12      /* float[n]     P of the last reorder (Eq. 28)                                */
+};
+
+/* Create a context.  Validates params, derives constants (m, B, alpha_D, eta^2, cell grid).
+ * Fails with SPH_E_BADARG on bad parameters, SPH_E_OVERFLOW if 2*ncells+2 does not fit 32 bits,
+ * SPH_E_CUDA if no CUDA device is usable. */
+int sph_create(const sph_params* params, sph_ctx** out);
+
+/* Release all device memory of the context.  NULL is allowed. */
+void sph_destroy(sph_ctx* ctx);
+
+/* Load n particles from host arrays (copied).  pos: double[n*3]; vel: float[n*3]; rho: float[n];
+ * type: uint8[n], 0 fluid, 1 fixed boundary, >= 2 moving-boundary group id (Eq. 37).
+ * Positions are converted on the device, in IEEE double, to the canonical state (C1):
+ * s = (x-min)/cs, c = floor(s), u = rint((s-c) 2^22) 2^-22 ("relative position of the
+ * particle within its cell (using single precision)").  Resets t, step count and counters.
+ * This is the one host->device crossing of the run. */
+int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, const float* vel,
+                       const float* rho, const uint8_t* type);
+
+/* Imposed motion of boundary group `group` (>= 2) along `axis` (Eq. 37):
+ * x(t) = x(0) + (stroke/2) (sin(2 pi t/period + phase) - sin(phase)), v = dx/dt. */
+int sph_set_motion(sph_ctx* ctx, int32_t group, int32_t axis, double stroke, double period,
+                   double phase);
+
+/* One neighbour-list build (cell key, radix sort, cell-range table, reorder) plus one
+ * particle-interaction pass (Eq. 15, 17-18, 21-22, 28, 36) on the current state.
+ * Results: SPH_ACC, SPH_DRHODT, SPH_NBCOUNT and the dt candidates of Eq. 35. */
+int sph_compute_interactions(sph_ctx* ctx);
+
+/* nsteps symplectic predictor-corrector steps (Eq. 33-34) with the variable dt of
+ * Eq. 35 taken from the pass at state n (A8).  Each step = 2 x (neighbour-list build + interaction
+ * pass) + dt reduction + predictor + corrector, all on the device, no host synchronisation. */
+int sph_step(sph_ctx* ctx, int32_t nsteps);
+
+/* Copy one field to host memory `dst` of `dst_bytes` bytes (must be at least the field's size, else
+ * SPH_E_OVERFLOW).  Synchronises the stream.  The other device->host crossing. */
+int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst_bytes);
+
+/* Fill *info (synchronises the stream). */
+int sph_get_info(sph_ctx* ctx, sph_info* info);
+
+/* Per-phase CUDA-event timing.  on = 1 starts (and clears) accumulation; on = 0 stops it.
+ * While on, every phase is bracketed by events on the context's stream. */
+int sph_set_profiling(sph_ctx* ctx, int32_t on);
+int sph_get_timings(sph_ctx* ctx, sph_timings* out);
+
+/* Message of the last error on this context ("" if none).  Valid until the next call. */
+const char* sph_last_error(const sph_ctx* ctx);
+
+/* Library version string, e.g. "sph_b200 0.1 (sm_100a)". */
+const char* sph_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

@@ -1,0 +1,587 @@
+// C ABI of libsph_b200.so (include/sph.h): host-side logic only -- parameter validation, derived
+// constants, device memory, the order of kernel launches for the NL -> PI -> SU loop of the paper
+// (Fig. 7), and the two host<->device crossings.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+#include <vector>
+
+#include "sph_internal.cuh"
+
+#define SPH_EXPORT extern "C" __attribute__((visibility("default")))
+
+enum Phase { PH_KEY = 0, PH_SORT, PH_CELLSTART, PH_REORDER, PH_PI, PH_DT, PH_UPDATE, PH_COUNT };
+
+struct EventPair {
+  int phase;
+  cudaEvent_t a, b;
+};
+
+struct sph_ctx {
+  sph_params prm;
+  DevConsts C;
+  cudaStream_t stream;
+  std::string err;
+  std::vector<void*> allocs;
+
+  int64_t n = 0, cap = 0;
+  bool loaded = false, nl_valid = false;
+  ParticleSet set[2];
+  int cur = 0;
+  float4* acc = nullptr;
+  uint32_t* nbcount = nullptr;
+  uint32_t *key[2] = {nullptr, nullptr}, *idx[2] = {nullptr, nullptr};
+  int sorted_buf = 0;
+  uint32_t *block_hist = nullptr, *digit_total = nullptr, *cellstart = nullptr;
+  uint32_t nkeys = 0;
+  int key_bits = 0;
+  DevScalars* sc = nullptr;
+  double* pos0 = nullptr;
+  bool has_moving = false;
+  std::vector<Motion> motions;
+  Motion* d_motions = nullptr;
+  int pi_kernel = 1;
+
+  bool profiling = false;
+  std::vector<EventPair> events;
+  std::vector<cudaEvent_t> pool;
+  double ms[PH_COUNT] = {0};
+  int64_t n_nl = 0, n_pi = 0, n_launch = 0;
+};
+
+namespace {
+
+int fail(sph_ctx* c, int code, const char* fmt, const char* detail = "") {
+  if (c) {
+    char buf[512];
+    snprintf(buf, sizeof(buf), fmt, detail);
+    c->err = buf;
+  }
+  return code;
+}
+
+int cuda_fail(sph_ctx* c, cudaError_t e, const char* where) {
+  if (c) c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? SPH_E_NOMEM : SPH_E_CUDA;
+}
+
+#define CK(call)                                                   \
+  do {                                                             \
+    cudaError_t e__ = (call);                                      \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);     \
+  } while (0)
+
+void* dalloc(sph_ctx* c, size_t bytes) {
+  if (bytes == 0) bytes = 16;
+  void* p = nullptr;
+  if (c->prm.dev_alloc) {
+    p = c->prm.dev_alloc(bytes, c->prm.user);
+  } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    p = nullptr;
+  }
+  if (p) c->allocs.push_back(p);
+  return p;
+}
+
+void dfree(sph_ctx* c, void* p) {
+  if (!p) return;
+  for (size_t i = 0; i < c->allocs.size(); i++)
+    if (c->allocs[i] == p) {
+      c->allocs.erase(c->allocs.begin() + i);
+      break;
+    }
+  if (c->prm.dev_free) c->prm.dev_free(p, c->prm.user);
+  else cudaFree(p);
+}
+
+void free_all(sph_ctx* c) {
+  while (!c->allocs.empty()) dfree(c, c->allocs.back());
+}
+
+// ---- profiling: one event pair per phase instance, folded into ms[] at synchronisation points ----
+cudaEvent_t get_event(sph_ctx* c) {
+  if (!c->pool.empty()) {
+    cudaEvent_t e = c->pool.back();
+    c->pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e;
+  cudaEventCreate(&e);
+  return e;
+}
+
+void fold_events(sph_ctx* c) {
+  if (c->events.empty()) return;
+  cudaStreamSynchronize(c->stream);
+  for (auto& ev : c->events) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, ev.a, ev.b) == cudaSuccess) c->ms[ev.phase] += t;
+    c->pool.push_back(ev.a);
+    c->pool.push_back(ev.b);
+  }
+  c->events.clear();
+}
+
+struct PhaseTimer {
+  sph_ctx* c;
+  EventPair ev;
+  bool on;
+  PhaseTimer(sph_ctx* ctx, int phase) : c(ctx), on(ctx->profiling) {
+    if (!on) return;
+    ev.phase = phase;
+    ev.a = get_event(c);
+    ev.b = get_event(c);
+    cudaEventRecord(ev.a, c->stream);
+  }
+  ~PhaseTimer() {
+    if (!on) return;
+    cudaEventRecord(ev.b, c->stream);
+    c->events.push_back(ev);
+    if (c->events.size() >= 8192) fold_events(c);
+  }
+};
+
+int validate(const sph_params* p, std::string& why) {
+  auto bad = [&](const char* s) { why = s; return SPH_E_BADARG; };
+  if (p->dim != 2 && p->dim != 3) return bad("dim must be 2 or 3");
+  if (!(p->dp > 0) || !(p->h > 0)) return bad("dp and h must be positive");
+  if (!(p->rho0 > 0) || !(p->c0 > 0) || !(p->gamma > 0)) return bad("rho0, c0, gamma must be positive");
+  if (!(p->cfl > 0)) return bad("cfl must be positive");
+  if (p->alpha < 0 || p->delta < 0 || p->eta2_coef < 0) return bad("alpha, delta, eta2_coef must be >= 0");
+  if (p->cell_div < 1 || p->cell_div > 3) return bad("cell_div must be 1, 2 or 3");
+  if (p->pi_kernel < 0 || p->pi_kernel > 2) return bad("pi_kernel must be 0, 1 or 2");
+  const double cs_min = 2.0 * p->h / p->cell_div;
+  if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
+  for (int k = 0; k < 3; k++) {
+    if (p->dim == 2 && k == 1) continue;
+    if (!(p->domain_max[k] > p->domain_min[k])) return bad("domain_max must exceed domain_min");
+  }
+  if ((p->dev_alloc == nullptr) != (p->dev_free == nullptr)) return bad("dev_alloc and dev_free must be given together");
+  return SPH_OK;
+}
+
+// Derived constants: m = rho0 dp^d (A9), B = c0^2 rho0/gamma (Eq. 28),
+// alpha_D (Eq. 11), eta^2 = eta2_coef h^2 (A6), grid n_k = ceil((max-min)/cs) (C3).
+int derive(const sph_params* p, DevConsts& C, std::string& why) {
+  const double pi = 3.14159265358979323846;
+  memset(&C, 0, sizeof(C));
+  C.dim = p->dim;
+  C.k = p->cell_div;
+  const double cs = p->cell_size > 0.0 ? p->cell_size : 2.0 * p->h / (double)p->cell_div;
+  C.cs = cs;
+  double ncells = 1.0;
+  for (int k = 0; k < 3; k++) {
+    C.per[k] = p->periodic[k] ? 1 : 0;
+    C.dmin[k] = p->domain_min[k];
+    if (p->dim == 2 && k == 1) { C.nc[k] = 1; C.per[k] = 0; continue; }
+    double ext = (p->domain_max[k] - p->domain_min[k]) / cs;
+    double nk = ceil(ext - 1e-9);
+    if (nk < 1) nk = 1;
+    if (nk > 2.0e9) { why = "grid too large"; return SPH_E_OVERFLOW; }
+    C.nc[k] = (int)nk;
+    ncells *= nk;
+    if (C.per[k] && C.nc[k] < 2 * C.k + 1) { why = "periodic axis needs at least 2*cell_div+1 cells"; return SPH_E_BADARG; }
+  }
+  if (2.0 * ncells + 2.0 >= 4294967295.0 || ncells >= 2147483647.0) { why = "2*ncells+2 does not fit 32-bit keys"; return SPH_E_OVERFLOW; }
+  C.ncells = (uint32_t)ncells;
+  const double s = 2.0 * p->h / cs;
+  C.R2u = (float)(s * s);
+  C.qscale = (float)(cs / (2.0 * p->h));
+  const double eta2 = p->eta2_coef * p->h * p->h;
+  C.eta2u = (float)(eta2 / (cs * cs));
+  C.rho0 = (float)p->rho0;
+  C.inv_rho0 = (float)(1.0 / p->rho0);
+  C.Beos = (float)(p->c0 * p->c0 * p->rho0 / p->gamma);
+  C.gamma = (float)p->gamma;
+  C.gamma_is7 = p->gamma == 7.0;
+  for (int k = 0; k < 3; k++) C.g[k] = (float)p->g[k];
+  const double m = p->rho0 * pow(p->dp, p->dim);
+  const double aD = p->dim == 2 ? 7.0 / (4.0 * pi * p->h * p->h) : 21.0 / (16.0 * pi * p->h * p->h * p->h);
+  const double Cf = -5.0 * aD / (p->h * p->h);     // grad_a W_ab = Cf (1 - q/2)^3 r_ab
+  C.c_cont = (float)(m * cs * Cf);
+  C.c_ddt = (float)(2.0 * p->delta * p->h * p->c0 * m * Cf);
+  C.c_mom = (float)(-m * Cf * cs);
+  C.c_pi = (float)(-2.0 * p->alpha * p->c0 * (p->h / cs));
+  C.c_mu = (float)(p->h / cs);
+  C.ddt_over_boundary = p->ddt_over_boundary;
+  C.rho_bound_floor = p->rho_bound_floor;
+  C.h = p->h;
+  C.c0 = p->c0;
+  C.cfl = p->cfl;
+  C.inv_cs = (float)(1.0 / cs);
+  return SPH_OK;
+}
+
+int alloc_set(sph_ctx* c, ParticleSet& P, int64_t n) {
+  P.posu = (float4*)dalloc(c, sizeof(float4) * n);
+  P.velp = (float4*)dalloc(c, sizeof(float4) * n);
+  P.cell = (int*)dalloc(c, sizeof(int) * n);
+  P.id = (uint32_t*)dalloc(c, sizeof(uint32_t) * n);
+  P.type = (uint8_t*)dalloc(c, n);
+  P.posu_n = (float4*)dalloc(c, sizeof(float4) * n);
+  P.vel_n = (float4*)dalloc(c, sizeof(float4) * n);
+  P.cell_n = (int*)dalloc(c, sizeof(int) * n);
+  return (P.posu && P.velp && P.cell && P.id && P.type && P.posu_n && P.vel_n && P.cell_n) ? 0 : -1;
+}
+
+// NL task: a1 key -> a2 sort -> a3 cell ranges -> a4 reorder (+a7 EOS)
+int build_nl(sph_ctx* ctx, bool with_n_state) {
+  const int64_t n = ctx->n;
+  cudaStream_t s = ctx->stream;
+  {
+    PhaseTimer t(ctx, PH_KEY);
+    nl_compute_keys(ctx->C, ctx->set[ctx->cur], n, ctx->key[0], ctx->idx[0], s);
+    ctx->n_launch += 1;
+  }
+  {
+    PhaseTimer t(ctx, PH_SORT);
+    int nl = 0;
+    ctx->sorted_buf = nl_radix_sort(ctx->key[0], ctx->idx[0], ctx->key[1], ctx->idx[1], n, ctx->key_bits,
+                                    ctx->block_hist, ctx->digit_total, &nl, s);
+    ctx->n_launch += nl;
+  }
+  {
+    PhaseTimer t(ctx, PH_CELLSTART);
+    nl_cellstart(ctx->key[ctx->sorted_buf], n, ctx->nkeys, ctx->cellstart, s);
+    ctx->n_launch += 1;
+  }
+  {
+    PhaseTimer t(ctx, PH_REORDER);
+    nl_reorder(ctx->C, ctx->set[ctx->cur], ctx->set[1 - ctx->cur], ctx->idx[ctx->sorted_buf], n, with_n_state, s);
+    ctx->cur = 1 - ctx->cur;
+    ctx->n_launch += 1;
+  }
+  ctx->n_nl += 1;
+  ctx->nl_valid = true;
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+// PI task: a5/a6 (+ dt candidates for a8)
+int run_pi(sph_ctx* ctx) {
+  cudaStream_t s = ctx->stream;
+  PhaseTimer t(ctx, PH_PI);
+  pi_reset_scalars(ctx->sc, s);
+  PiArgs A;
+  const ParticleSet& P = ctx->set[ctx->cur];
+  A.posu = P.posu;
+  A.velp = P.velp;
+  A.cell = P.cell;
+  A.cellstart = ctx->cellstart;
+  A.acc = ctx->acc;
+  A.nbcount = ctx->prm.count_neighbours ? ctx->nbcount : nullptr;
+  A.sc = ctx->sc;
+  A.n = ctx->n;
+  bool done = false;
+  if (ctx->pi_kernel == 2) done = pi_tiled(ctx->C, A, s) == 0;
+  if (!done) pi_gather(ctx->C, A, s);
+  ctx->n_launch += 2;
+  ctx->n_pi += 1;
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+int check_flags(sph_ctx* ctx, const DevScalars& h) {
+  if (h.flags & 1u) return fail(ctx, SPH_E_NAN, "non-finite acceleration or density rate detected on the device");
+  if (h.flags & 2u) return fail(ctx, SPH_E_OVERFLOW, "device-side overflow");
+  return SPH_OK;
+}
+
+}  // namespace
+
+SPH_EXPORT const char* sph_version(void) { return "sph_b200 0.1 (sm_100a)"; }
+
+SPH_EXPORT const char* sph_last_error(const sph_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
+  if (!params || !out) return SPH_E_BADARG;
+  *out = nullptr;
+  std::string why;
+  int rc = validate(params, why);
+  if (rc != SPH_OK) return rc;
+  sph_ctx* ctx = new (std::nothrow) sph_ctx();
+  if (!ctx) return SPH_E_NOMEM;
+  ctx->prm = *params;
+  rc = derive(params, ctx->C, why);
+  if (rc != SPH_OK) { delete ctx; return rc; }
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {       // no CPU fallback: fail loudly
+    cudaGetLastError();
+    delete ctx;
+    return SPH_E_CUDA;
+  }
+  ctx->stream = (cudaStream_t)params->cuda_stream;
+  ctx->nkeys = 2u * ctx->C.ncells + 1u;      // keys 0 .. 2*ncells (C3)
+  ctx->key_bits = 0;
+  for (uint32_t v = 2u * ctx->C.ncells; v; v >>= 1) ctx->key_bits++;
+  if (ctx->key_bits == 0) ctx->key_bits = 1;
+  ctx->pi_kernel = params->pi_kernel == 0 ? 1 : params->pi_kernel;
+  ctx->cellstart = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * ((size_t)ctx->nkeys + 1));
+  ctx->sc = (DevScalars*)dalloc(ctx, sizeof(DevScalars));
+  ctx->digit_total = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * 256 * 4);
+  if (!ctx->cellstart || !ctx->sc || !ctx->digit_total) {
+    free_all(ctx);
+    delete ctx;
+    return SPH_E_NOMEM;
+  }
+  if (cudaMemsetAsync(ctx->sc, 0, sizeof(DevScalars), ctx->stream) != cudaSuccess) {
+    free_all(ctx);
+    delete ctx;
+    return SPH_E_CUDA;
+  }
+  *out = ctx;
+  return SPH_OK;
+}
+
+SPH_EXPORT void sph_destroy(sph_ctx* ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  for (auto& ev : ctx->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+  for (auto e : ctx->pool) cudaEventDestroy(e);
+  free_all(ctx);
+  delete ctx;
+}
+
+SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, const float* vel, const float* rho,
+                                  const uint8_t* type) {
+  if (!ctx) return SPH_E_BADARG;
+  if (n < 0 || n > 0x7fffffff - 8192) return fail(ctx, SPH_E_BADARG, "n out of range");
+  if (n > 0 && (!pos || !vel || !rho || !type)) return fail(ctx, SPH_E_BADARG, "null input array");
+  cudaStream_t s = ctx->stream;
+  if (n > ctx->cap || !ctx->acc) {            // (re)allocate particle storage
+    cudaStreamSynchronize(s);
+    void* keep[] = {ctx->cellstart, ctx->sc, ctx->digit_total, ctx->d_motions};
+    std::vector<void*> old = ctx->allocs;
+    for (void* p : old) {
+      bool k = false;
+      for (void* q : keep) k = k || (p == q);
+      if (!k) dfree(ctx, p);
+    }
+    ctx->cap = 0;
+    const int64_t cap = n;
+    bool ok = alloc_set(ctx, ctx->set[0], cap) == 0 && alloc_set(ctx, ctx->set[1], cap) == 0;
+    ctx->acc = (float4*)dalloc(ctx, sizeof(float4) * cap);
+    ctx->nbcount = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * cap);
+    for (int i = 0; i < 2; i++) {
+      ctx->key[i] = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * cap);
+      ctx->idx[i] = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * cap);
+    }
+    ctx->block_hist = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * nl_radix_hist_entries(cap));
+    ctx->pos0 = nullptr;
+    ok = ok && ctx->acc && ctx->nbcount && ctx->key[0] && ctx->key[1] && ctx->idx[0] && ctx->idx[1] && ctx->block_hist;
+    if (!ok) return fail(ctx, SPH_E_NOMEM, "device allocation failed for %s particles", std::to_string(n).c_str());
+    ctx->cap = cap;
+  }
+  ctx->has_moving = false;
+  for (int64_t i = 0; i < n; i++)
+    if (type[i] >= 2) { ctx->has_moving = true; break; }
+  if (ctx->has_moving && !ctx->pos0) {
+    ctx->pos0 = (double*)dalloc(ctx, sizeof(double) * 3 * ctx->cap);
+    if (!ctx->pos0) return fail(ctx, SPH_E_NOMEM, "device allocation failed (pos0)");
+  }
+  // staging buffers for the raw inputs
+  double* d_pos = (double*)dalloc(ctx, sizeof(double) * 3 * n);
+  float* d_vel = (float*)dalloc(ctx, sizeof(float) * 3 * n);
+  float* d_rho = (float*)dalloc(ctx, sizeof(float) * n);
+  uint8_t* d_type = (uint8_t*)dalloc(ctx, n);
+  if (!d_pos || !d_vel || !d_rho || !d_type) return fail(ctx, SPH_E_NOMEM, "device allocation failed (staging)");
+  CK(cudaMemsetAsync(ctx->sc, 0, sizeof(DevScalars), s));
+  if (n > 0) {
+    CK(cudaMemcpyAsync(d_pos, pos, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(d_vel, vel, sizeof(float) * 3 * n, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(d_rho, rho, sizeof(float) * n, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(d_type, type, n, cudaMemcpyHostToDevice, s));
+  }
+  ctx->cur = 0;
+  su_canonicalize(ctx->C, d_pos, d_vel, d_rho, d_type, n, ctx->set[0], ctx->has_moving ? ctx->pos0 : nullptr,
+                  ctx->sc, s);
+  ctx->n_launch += 1;
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(s));
+  dfree(ctx, d_pos);
+  dfree(ctx, d_vel);
+  dfree(ctx, d_rho);
+  dfree(ctx, d_type);
+  ctx->n = n;
+  ctx->loaded = true;
+  ctx->nl_valid = false;
+  return SPH_OK;
+}
+
+SPH_EXPORT int sph_set_motion(sph_ctx* ctx, int32_t group, int32_t axis, double stroke, double period, double phase) {
+  if (!ctx) return SPH_E_BADARG;
+  if (group < 2 || group > 255) return fail(ctx, SPH_E_BADARG, "motion group must be in 2..255");
+  if (axis < 0 || axis > 2 || !(period > 0)) return fail(ctx, SPH_E_BADARG, "bad axis or period");
+  Motion m = {group, axis, stroke, period, phase};
+  bool found = false;
+  for (auto& q : ctx->motions)
+    if (q.group == group && q.axis == axis) { q = m; found = true; }
+  if (!found) ctx->motions.push_back(m);
+  if (ctx->d_motions) { cudaStreamSynchronize(ctx->stream); dfree(ctx, ctx->d_motions); }
+  ctx->d_motions = (Motion*)dalloc(ctx, sizeof(Motion) * ctx->motions.size());
+  if (!ctx->d_motions) return fail(ctx, SPH_E_NOMEM, "device allocation failed (motions)");
+  CK(cudaMemcpyAsync(ctx->d_motions, ctx->motions.data(), sizeof(Motion) * ctx->motions.size(),
+                     cudaMemcpyHostToDevice, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  return SPH_OK;
+}
+
+SPH_EXPORT int sph_compute_interactions(sph_ctx* ctx) {
+  if (!ctx) return SPH_E_BADARG;
+  if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_compute_interactions before sph_load_particles");
+  int rc = build_nl(ctx, false);
+  if (rc != SPH_OK) return rc;
+  rc = run_pi(ctx);
+  if (rc != SPH_OK) return rc;
+  {
+    PhaseTimer t(ctx, PH_DT);
+    su_compute_dt(ctx->C, ctx->sc, ctx->stream);
+    ctx->n_launch += 1;
+  }
+  return SPH_OK;
+}
+
+SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
+  if (!ctx) return SPH_E_BADARG;
+  if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_step before sph_load_particles");
+  if (nsteps < 0) return fail(ctx, SPH_E_BADARG, "nsteps < 0");
+  cudaStream_t s = ctx->stream;
+  const int nm = ctx->has_moving ? (int)ctx->motions.size() : 0;
+  for (int it = 0; it < nsteps; it++) {
+    int rc;
+    if ((rc = build_nl(ctx, false)) != SPH_OK) return rc;        // NL at state n
+    if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^n, R^n
+    {
+      PhaseTimer t(ctx, PH_DT);
+      su_compute_dt(ctx->C, ctx->sc, s);                         // dt^n (Eq. 35, A8)
+      ctx->n_launch += 1;
+    }
+    {
+      PhaseTimer t(ctx, PH_UPDATE);
+      su_predictor(ctx->C, ctx->set[ctx->cur], ctx->acc, ctx->n, ctx->sc, ctx->d_motions, nm, ctx->pos0, s);
+      ctx->n_launch += 1;
+    }
+    if ((rc = build_nl(ctx, true)) != SPH_OK) return rc;         // NL at state n+1/2
+    if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^{n+1/2}, R^{n+1/2}
+    {
+      PhaseTimer t(ctx, PH_UPDATE);
+      su_corrector(ctx->C, ctx->set[ctx->cur], ctx->acc, ctx->n, ctx->sc, ctx->d_motions, nm, ctx->pos0, s);
+      ctx->n_launch += 2;
+    }
+    ctx->nl_valid = false;   // positions moved after the last build
+    CK(cudaGetLastError());
+  }
+  return SPH_OK;
+}
+
+SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst_bytes) {
+  if (!ctx || !dst) return SPH_E_BADARG;
+  if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_read_state before sph_load_particles");
+  const int64_t n = ctx->n;
+  cudaStream_t s = ctx->stream;
+  const ParticleSet& P = ctx->set[ctx->cur];
+  size_t need = 0;
+  switch (field) {
+    case SPH_POS: need = sizeof(double) * 3 * n; break;
+    case SPH_VEL: case SPH_ACC: case SPH_OFFSET: need = sizeof(float) * 3 * n; break;
+    case SPH_RHO: case SPH_DRHODT: case SPH_PRESS: need = sizeof(float) * n; break;
+    case SPH_KEY: case SPH_PERM: case SPH_NBCOUNT: need = sizeof(uint32_t) * n; break;
+    case SPH_CELL: need = sizeof(int32_t) * 3 * n; break;
+    case SPH_CELLSTART: need = sizeof(uint32_t) * ((size_t)ctx->nkeys + 1); break;
+    default: return fail(ctx, SPH_E_BADARG, "unknown field");
+  }
+  if (dst_bytes < need) return fail(ctx, SPH_E_OVERFLOW, "destination buffer too small");
+  if ((field == SPH_KEY || field == SPH_CELLSTART || field == SPH_ACC || field == SPH_DRHODT ||
+       field == SPH_NBCOUNT) && ctx->n_nl == 0)
+    return fail(ctx, SPH_E_STATE, "field needs a neighbour-list build / interaction pass first");
+  if (field == SPH_NBCOUNT && !ctx->prm.count_neighbours)
+    return fail(ctx, SPH_E_STATE, "SPH_NBCOUNT needs params.count_neighbours = 1");
+  if (need == 0) return SPH_OK;
+  if (field == SPH_KEY) {
+    CK(cudaMemcpyAsync(dst, ctx->key[ctx->sorted_buf], need, cudaMemcpyDeviceToHost, s));
+  } else if (field == SPH_PERM) {
+    CK(cudaMemcpyAsync(dst, P.id, need, cudaMemcpyDeviceToHost, s));
+  } else if (field == SPH_CELLSTART) {
+    CK(cudaMemcpyAsync(dst, ctx->cellstart, need, cudaMemcpyDeviceToHost, s));
+  } else {
+    void* tmp = dalloc(ctx, need);
+    if (!tmp) return fail(ctx, SPH_E_NOMEM, "device allocation failed (read buffer)");
+    switch (field) {
+      case SPH_POS: su_unsort_pos(ctx->C, P, n, (double*)tmp, nullptr, nullptr, s); break;
+      case SPH_CELL: su_unsort_pos(ctx->C, P, n, nullptr, (int*)tmp, nullptr, s); break;
+      case SPH_OFFSET: su_unsort_pos(ctx->C, P, n, nullptr, nullptr, (float*)tmp, s); break;
+      case SPH_VEL: su_unsort_f4(P.velp, P.id, n, 3, 0, (float*)tmp, s); break;
+      case SPH_PRESS: su_unsort_f4(P.velp, P.id, n, 1, 3, (float*)tmp, s); break;
+      case SPH_RHO: su_unsort_f4(P.posu, P.id, n, 1, 3, (float*)tmp, s); break;
+      case SPH_ACC: su_unsort_f4(ctx->acc, P.id, n, 3, 0, (float*)tmp, s); break;
+      case SPH_DRHODT: su_unsort_f4(ctx->acc, P.id, n, 1, 3, (float*)tmp, s); break;
+      case SPH_NBCOUNT: su_unsort_u32(ctx->nbcount, P.id, n, (uint32_t*)tmp, s); break;
+    }
+    ctx->n_launch += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dst, tmp, need, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    dfree(ctx, tmp);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "sph_read_state");
+  }
+  CK(cudaStreamSynchronize(s));
+  return SPH_OK;
+}
+
+SPH_EXPORT int sph_get_info(sph_ctx* ctx, sph_info* info) {
+  if (!ctx || !info) return SPH_E_BADARG;
+  DevScalars h;
+  CK(cudaMemcpyAsync(&h, ctx->sc, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+  uint32_t nb = 0;
+  if (ctx->n_nl > 0) CK(cudaMemcpyAsync(&nb, ctx->cellstart + ctx->C.ncells, sizeof(nb), cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  memset(info, 0, sizeof(*info));
+  info->n = ctx->n;
+  info->n_out = h.n_out;
+  info->n_bound = nb;
+  for (int k = 0; k < 3; k++) info->ncell[k] = ctx->C.nc[k];
+  info->ncells = ctx->C.ncells;
+  info->cell_size = ctx->C.cs;
+  info->r2u = ctx->C.R2u;
+  info->n_interactions = h.n_inter;
+  info->n_interactions_total = h.n_inter_total + h.n_inter;
+  info->steps_done = (int64_t)h.steps;
+  info->t = h.t;
+  info->dt = h.dt;
+  info->pi_kernel = ctx->pi_kernel;
+  info->device_flags = (int32_t)h.flags;
+  return check_flags(ctx, h);
+}
+
+SPH_EXPORT int sph_set_profiling(sph_ctx* ctx, int32_t on) {
+  if (!ctx) return SPH_E_BADARG;
+  fold_events(ctx);
+  if (on) {
+    for (int i = 0; i < PH_COUNT; i++) ctx->ms[i] = 0.0;
+    ctx->n_nl = ctx->n_nl;  // counters keep running; timings restart
+  }
+  ctx->profiling = on != 0;
+  return SPH_OK;
+}
+
+SPH_EXPORT int sph_get_timings(sph_ctx* ctx, sph_timings* out) {
+  if (!ctx || !out) return SPH_E_BADARG;
+  fold_events(ctx);
+  CK(cudaStreamSynchronize(ctx->stream));
+  out->ms_key = ctx->ms[PH_KEY];
+  out->ms_sort = ctx->ms[PH_SORT];
+  out->ms_cellstart = ctx->ms[PH_CELLSTART];
+  out->ms_reorder = ctx->ms[PH_REORDER];
+  out->ms_interaction = ctx->ms[PH_PI];
+  out->ms_dt = ctx->ms[PH_DT];
+  out->ms_update = ctx->ms[PH_UPDATE];
+  out->n_nl_builds = ctx->n_nl;
+  out->n_interaction_passes = ctx->n_pi;
+  out->n_kernel_launches = ctx->n_launch;
+  return SPH_OK;
+}

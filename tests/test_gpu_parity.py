@@ -1,0 +1,287 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star):
+  * bit-exact: canonical state (C1), cell keys, sort permutation, cell ranges, per-particle
+    neighbour counts (C2/C3);
+  * relative 1e-4 with absolute floor 1e-6 * max|value| for per-particle acceleration and drho/dt
+    after one interaction call;
+  * after 10 steps: particle count conserved, total density sum within 1e-6 relative, per-particle
+    position error <= 1e-3 dp.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2104_00537_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [1, 2]  # 1 = gather (thread per particle), 2 = tiled shared-memory kernel
+
+
+@pytest.fixture(scope="module")
+def sph():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2104_00537_b200 import sph as mod
+    return mod
+
+
+def assert_close(name, got, ref, rtol=1e-4, floor=1e-6):
+    got = np.asarray(got, np.float64)
+    ref = np.asarray(ref, np.float64)
+    scale = np.abs(ref).max() if ref.size else 0.0
+    err = np.abs(got - ref)
+    tol = rtol * np.abs(ref) + floor * scale
+    bad = err > tol
+    assert not bad.any(), (f"{name}: {bad.sum()} of {bad.size} outside rel {rtol} / floor {floor}*{scale:.3e}; "
+                           f"worst err {err.max():.3e} at {np.unravel_index(err.argmax(), err.shape)} "
+                           f"(ref {ref.ravel()[err.argmax()]:.6e})")
+
+
+def check_one_pass(sph, case, pi_kernel, check_perm=True):
+    """load -> sph_compute_interactions -> compare every output with the oracle."""
+    p = case.params
+    st = oracle.State(p, case.pos, case.vel, case.rho, case.ptype)
+    ref = st.interactions(mode=1)
+    key, perm, cellstart = oracle.neighbour_list(p, st.cell, st.u, st.ptype, st.out)
+    with sph.Sph(p, pi_kernel=pi_kernel, count_neighbours=True) as S:
+        S.load_case(case)
+        # C1: canonical state
+        assert np.array_equal(S.read_state(sph.SPH_OFFSET)[st.out == 0], st.u[st.out == 0])
+        cell = S.read_state(sph.SPH_CELL)
+        assert np.array_equal(cell[st.out == 0], st.cell[st.out == 0])
+        assert (cell[st.out == 1] == -1).all()
+        S.compute_interactions()
+        info = S.get_info()
+        assert info.n_out == int(st.out.sum())
+        assert tuple(info.ncell) == oracle.grid(p)[1]
+        assert np.float32(info.r2u) == oracle.grid(p)[2]
+        # C3: keys, order, ranges -- bit exact
+        assert np.array_equal(S.read_state(sph.SPH_KEY), key[perm])
+        if check_perm:
+            assert np.array_equal(S.read_state(sph.SPH_PERM), perm)
+        assert np.array_equal(S.read_state(sph.SPH_CELLSTART), cellstart)
+        # C2: neighbour counts -- bit exact
+        nb = S.read_state(sph.SPH_NBCOUNT)
+        act = st.out == 0
+        assert np.array_equal(nb[act], ref["nbcount"][act])
+        assert info.n_interactions == int(ref["nbcount"].sum())
+        # Eq. 15/22/36 sums
+        assert_close("acc", S.read_state(sph.SPH_ACC)[act], ref["acc"][act])
+        assert_close("drho", S.read_state(sph.SPH_DRHODT)[act], ref["drho"][act])
+        # Eq. 35
+        dt_ref = oracle.dt(p, ref["acc"], st.ptype, st.out, ref["viscmax"])
+        assert info.dt == pytest.approx(dt_ref, rel=1e-5)
+        # Eq. 28
+        P_ref = np.array([oracle.eos(p, float(r)) for r in st.rho[:2000]])
+        assert_close("P", S.read_state(sph.SPH_PRESS)[:2000][act[:2000]], P_ref[act[:2000]], rtol=2e-6, floor=1e-9)
+        assert info.pi_kernel in (1, 2)
+        return info
+
+
+def developed_state(case, nsteps):
+    """Advance with the ORACLE, then round v, rho to fp32: a non-trivial state as a new input case."""
+    st = oracle.State(case.params, case.pos, case.vel, case.rho, case.ptype)
+    st.step(nsteps)
+    return wl.Case(case.name + f"_dev{nsteps}", st.pos, st.vel.astype(np.float32), st.rho.astype(np.float32),
+                   case.ptype.copy(), dict(case.params))
+
+
+# ---- one interaction call ------------------------------------------------------------------------------
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+@pytest.mark.parametrize("cell_div", [1, 2])
+def test_config0_initial_state(sph, pi_kernel, cell_div):
+    info = check_one_pass(sph, wl.config(0, cell_div=cell_div), pi_kernel)
+    assert info.n_interactions == 1738918
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+@pytest.mark.parametrize("cell_div", [1, 2])
+def test_config0_developed_state(sph, pi_kernel, cell_div):
+    case = developed_state(wl.config(0, cell_div=cell_div), 12)
+    check_one_pass(sph, case, pi_kernel)
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_config0_shuffled_load_order(sph, pi_kernel):
+    c = wl.dam_break("cfg0s", 3, 0.02, (50, 25, 25), (15, 25, 15), 0.01, 1234, 0.3, shuffle=True)
+    check_one_pass(sph, developed_state(c, 3), pi_kernel)
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+@pytest.mark.parametrize("dim,periodic,cell_div,n", [
+    (3, (0, 0, 0), 1, 20011), (3, (1, 1, 1), 1, 20011), (3, (1, 1, 1), 2, 9973), (3, (0, 0, 0), 2, 9973),
+    (2, (0, 0, 0), 1, 6007), (2, (1, 0, 1), 1, 6007), (2, (1, 0, 1), 2, 6007), (3, (0, 0, 0), 3, 5003)])
+def test_random_clouds(sph, pi_kernel, dim, periodic, cell_div, n):
+    box = (0.9, 0.9 if dim == 3 else 0.0, 0.9) if dim == 3 else (2.4, 0.0, 2.4)
+    c = wl.random_cloud("rc", n, box, 0.02, 1000 + dim * 10 + cell_div + sum(periodic), dim=dim,
+                        periodic=periodic, cell_div=cell_div)
+    check_one_pass(sph, c, pi_kernel)
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+@pytest.mark.parametrize("cell_div", [1, 2])
+def test_config3_periodic_cloud_scaled(sph, pi_kernel, cell_div):
+    c = wl.config(3, cell_div=cell_div, scale=40 / 252)   # 40^3 = 64 k particles, same recipe
+    info = check_one_pass(sph, c, pi_kernel)
+    assert info.n_interactions > 280 * c.n
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+@pytest.mark.parametrize("cell_div", [1, 2])
+def test_config1_dambreak2d_scaled(sph, pi_kernel, cell_div):
+    c = wl.config(1, cell_div=cell_div, scale=0.1)         # ~10 k fluid particles, 2-D
+    check_one_pass(sph, developed_state(c, 6), pi_kernel)
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_config2_dambreak3d_scaled(sph, pi_kernel):
+    c = wl.config(2, scale=0.2)                            # ~33 k fluid + boundaries, same geometry
+    check_one_pass(sph, developed_state(c, 3), pi_kernel)
+
+
+# ---- edge cases ---------------------------------------------------------------------------------------
+def small_params(**kw):
+    p = wl._params(3, 0.02, 1.2, 17.0, (0, 0, -9.81), (0, 0, 0), (0.5, 0.5, 0.5))
+    p.update(kw)
+    return p
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_empty_and_single_particle(sph, pi_kernel):
+    p = small_params()
+    with sph.Sph(p, pi_kernel=pi_kernel, count_neighbours=True) as S:
+        S.load_particles(np.zeros((0, 3)), np.zeros((0, 3), np.float32), np.zeros(0, np.float32), np.zeros(0, np.uint8))
+        S.compute_interactions()
+        S.step(2)
+        assert S.get_info().n_interactions == 0
+        assert (S.read_state(sph.SPH_CELLSTART) == 0).all()
+        S.load_particles(np.array([[0.25, 0.25, 0.4]]), np.zeros((1, 3), np.float32), np.array([1000.0], np.float32),
+                         np.zeros(1, np.uint8))
+        S.compute_interactions()
+        assert S.read_state(sph.SPH_NBCOUNT)[0] == 0
+        np.testing.assert_allclose(S.read_state(sph.SPH_ACC)[0], [0, 0, -9.81], rtol=1e-6)
+        S.step(3)   # free fall: z = z0 - g t^2 / 2
+        t = S.get_info().t
+        np.testing.assert_allclose(S.read_state(sph.SPH_POS)[0], [0.25, 0.25, 0.4 - 0.5 * 9.81 * t * t], atol=1e-6)
+        np.testing.assert_allclose(S.read_state(sph.SPH_VEL)[0], [0, 0, -9.81 * t], rtol=1e-5)
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_all_boundary_and_out_of_grid(sph, pi_kernel):
+    c = wl.random_cloud("rc", 3001, (0.5, 0.5, 0.5), 0.02, 5)
+    c.ptype[:] = 1                                        # boundary only: no pair is evaluated (Eq. 36)
+    info = check_one_pass(sph, c, pi_kernel)
+    assert info.n_interactions == 0
+    c = wl.random_cloud("rc", 3001, (0.5, 0.5, 0.5), 0.02, 6)
+    c.pos[::7, 0] += 5.0                                  # every 7th particle outside the grid (A16)
+    c.pos[3, 2] = -3.0
+    info = check_one_pass(sph, c, pi_kernel)
+    assert info.n_out == len(c.pos[::7]) + (0 if 3 % 7 == 0 else 1)
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_crowded_cells_and_coincident_particles(sph, pi_kernel):
+    # 4000 particles in a 2.5-cell blob (hundreds per cell) + exact duplicates (r = 0, A17)
+    p = small_params()
+    n = 4000
+    idx = np.arange(n)
+    pos = 0.2 + 0.1 * np.stack([wl.uniform01(9, idx, k) for k in range(3)], 1)
+    pos[100:120] = pos[200:220]                           # coincident distinct pairs
+    vel = (0.3 * np.stack([wl.normal01(9, idx, 3 + k) for k in range(3)], 1)).astype(np.float32)
+    rho = (1000 * (1 + 0.01 * wl.normal01(9, idx, 6))).astype(np.float32)
+    typ = (wl.uniform01(9, idx, 7) < 0.3).astype(np.uint8)
+    c = wl.Case("blob", pos, vel, rho, typ, p)
+    info = check_one_pass(sph, c, pi_kernel)
+    assert info.n_interactions > 500 * n
+
+
+# ---- stepping ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+@pytest.mark.parametrize("cell_div", [1, 2])
+def test_config0_ten_steps(sph, pi_kernel, cell_div):
+    c = wl.config(0, cell_div=cell_div)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).step(10)
+    with sph.Sph(c.params, pi_kernel=pi_kernel) as S:
+        S.load_case(c)
+        S.step(10)
+        info = S.get_info()
+        assert info.steps_done == 10 and info.n_out == 0 and st.out.sum() == 0
+        assert info.t == pytest.approx(st.t, rel=1e-5)
+        pos = S.read_state(sph.SPH_POS)
+        err = np.abs(pos - st.pos).max()
+        assert err <= 1e-3 * c.params["dp"], err
+        rho = S.read_state(sph.SPH_RHO).astype(np.float64)
+        assert len(rho) == c.n                                           # particle count conserved (Eq. 14)
+        assert abs(rho.sum() - st.rho.sum()) <= 1e-6 * st.rho.sum()
+        assert_close("rho", rho, st.rho, rtol=1e-5, floor=0)
+        # velocities are not part of the stated tolerance; ten fp32 steps leave ~1e-5 |v|max of rounding
+        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-3, floor=1e-3)
+        # 2 builds + 2 passes per step
+        tm = S.get_timings()
+        assert tm.n_nl_builds == 20 and tm.n_interaction_passes == 20
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_periodic_cloud_steps_conserve_momentum(sph, pi_kernel):
+    c = wl.config(3, scale=24 / 252)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).step(5)
+    with sph.Sph(c.params, pi_kernel=pi_kernel) as S:
+        S.load_case(c)
+        S.step(5)
+        pos = S.read_state(sph.SPH_POS)
+        L = c.params["domain_max"][0]
+        d = np.abs(pos - st.pos)
+        d = np.minimum(d, L - d)                                        # periodic wrap
+        assert d.max() <= 1e-3 * c.params["dp"]
+        v = S.read_state(sph.SPH_VEL).astype(np.float64)
+        assert np.abs(v.sum(0) - c.vel.astype(np.float64).sum(0)).max() < 1e-4 * np.abs(v).sum()
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_moving_boundary_piston(sph, pi_kernel):
+    c = wl.wave_flume("flume_small", 0.05, 2.0, 0.3, 0.5, 0.3, 21, stroke=0.1, period=0.5, beach_slope=0.5)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype, motions=c.motions).step(6)
+    with sph.Sph(c.params, pi_kernel=pi_kernel) as S:
+        S.load_case(c)
+        S.step(6)
+        pos = S.read_state(sph.SPH_POS)
+        assert np.abs(pos - st.pos).max() <= 1e-3 * c.params["dp"]
+        mv = c.ptype >= 2
+        assert mv.sum() > 0
+        assert np.abs(pos[mv, 0] - c.pos[mv, 0]).min() > 1e-5          # the piston moved
+        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-3, floor=1e-3)
+
+
+def test_read_buffer_too_small_and_state_errors(sph):
+    import ctypes as C
+    p = small_params()
+    with sph.Sph(p) as S:
+        with pytest.raises(sph.SphError) as e:
+            S.step(1)
+        assert e.value.code == sph.SPH_E_STATE
+        S.load_particles(np.full((10, 3), 0.25), np.zeros((10, 3), np.float32), np.full(10, 1000.0, np.float32),
+                         np.zeros(10, np.uint8))
+        buf = np.zeros(5, np.float32)
+        with pytest.raises(sph.SphError) as e:
+            S.read_state_ptr(sph.SPH_RHO, buf.ctypes.data, buf.nbytes)
+        assert e.value.code == sph.SPH_E_OVERFLOW
+        with pytest.raises(sph.SphError) as e:
+            S.read_state(sph.SPH_NBCOUNT)
+        assert e.value.code == sph.SPH_E_STATE
+
+
+def test_nan_is_flagged(sph):
+    p = small_params()
+    with sph.Sph(p) as S:
+        rho = np.full(50, 1000.0, np.float32)
+        rho[7] = np.nan
+        pos = 0.2 + 0.05 * np.stack([wl.uniform01(1, np.arange(50), k) for k in range(3)], 1)
+        S.load_particles(pos, np.zeros((50, 3), np.float32), rho, np.zeros(50, np.uint8))
+        S.step(1)
+        with pytest.raises(sph.SphError) as e:
+            S.get_info()
+        assert e.value.code == sph.SPH_E_NAN
