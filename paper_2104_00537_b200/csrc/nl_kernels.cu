@@ -145,14 +145,18 @@ __global__ void __launch_bounds__(RS_THREADS) k_rs_scatter(const uint32_t* __res
   }
 }
 
-// a3: cellstart[k] = #{sorted keys < k}, k = 0 .. nkeys (nkeys + 1 entries)
+// a3: cellstart[k] = #{sorted keys < k}, k = 0 .. nkeys (nkeys + 1 entries): one lower-bound search per key,
+// so empty cells (most of a dam-break grid is air) cost the same as full ones.
 __global__ void k_cellstart(const uint32_t* __restrict__ key, int64_t n, uint32_t nkeys,
                             uint32_t* __restrict__ cellstart) {
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i > n) return;
-  int64_t prev = i == 0 ? -1 : (int64_t)key[i - 1];
-  int64_t cur = i == n ? (int64_t)nkeys : (int64_t)key[i];
-  for (int64_t k = prev + 1; k <= cur; k++) cellstart[k] = (uint32_t)i;
+  uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k > nkeys) return;
+  int64_t lo = 0, hi = n;            // first index with key[idx] >= k
+  while (lo < hi) {
+    int64_t mid = (lo + hi) >> 1;
+    if (key[mid] < k) lo = mid + 1; else hi = mid;
+  }
+  cellstart[k] = (uint32_t)lo;
 }
 
 // Tait EOS, Eq. 28, evaluated without the cancellation of (rho/rho0)^gamma - 1:
@@ -232,7 +236,7 @@ int nl_radix_sort(uint32_t* key_a, uint32_t* idx_a, uint32_t* key_b, uint32_t* i
 }
 
 void nl_cellstart(const uint32_t* sorted_key, int64_t n, uint32_t nkeys, uint32_t* cellstart, cudaStream_t s) {
-  k_cellstart<<<grid_for(n + 1, 256), 256, 0, s>>>(sorted_key, n, nkeys, cellstart);
+  k_cellstart<<<grid_for((int64_t)nkeys + 1, 256), 256, 0, s>>>(sorted_key, n, nkeys, cellstart);
 }
 
 void nl_reorder(const DevConsts& C, const ParticleSet& src, const ParticleSet& dst, const uint32_t* idx,

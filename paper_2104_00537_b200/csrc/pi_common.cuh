@@ -101,3 +101,81 @@ __device__ __forceinline__ void reduce_scalars(DevScalars* sc, float f2, float v
     if (nb) atomicAdd(&sc->n_inter, (unsigned long long)nb);
   }
 }
+
+// One particle a against the particles of its adjacent cells, read straight from global memory
+// (sorted arrays + cell-range table).  Used by the baseline kernel and as the overflow path of the tiled one.
+template <int DIM>
+__device__ __forceinline__ void gather_one(const DevConsts& C, const PiArgs& A, uint32_t a, bool a_fluid, float& f2,
+                                        float& visc, unsigned int& nb_out) {
+  const float4 pa = A.posu[a];
+  const float4 va = A.velp[a];
+  const int lin = A.cell[a];
+  int ca[3];
+  ca[0] = lin % C.nc[0];
+  int r = lin / C.nc[0];
+  ca[1] = r % C.nc[1];
+  ca[2] = r / C.nc[1];
+  const float inv_rho_a = fast_rcp(pa.w);
+  PairAcc S = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  unsigned int nb = 0;
+  const int K = C.k;
+  const int ky = DIM == 3 ? K : 0;
+  for (int dz = -K; dz <= K; dz++) {
+    int cz = ca[2] + dz;
+    if (C.per[2]) cz = (cz + C.nc[2]) % C.nc[2];
+    else if (cz < 0 || cz >= C.nc[2]) continue;
+    for (int dy = -ky; dy <= ky; dy++) {
+      int cy = ca[1] + dy;
+      if (C.per[1]) cy = (cy + C.nc[1]) % C.nc[1];
+      else if (cy < 0 || cy >= C.nc[1]) continue;
+      for (int dx = -K; dx <= K; dx++) {
+        int cx = ca[0] + dx;
+        if (C.per[0]) cx = (cx + C.nc[0]) % C.nc[0];
+        else if (cx < 0 || cx >= C.nc[0]) continue;
+        const uint32_t lin2 = (uint32_t)cx + (uint32_t)C.nc[0] * ((uint32_t)cy + (uint32_t)C.nc[1] * (uint32_t)cz);
+        // offsets of a relative to the neighbour cell's origin: du = ua - (ub + dc)  (exact, C1)
+        const float ox = pa.x - (float)dx, oy = pa.y - (float)dy, oz = pa.z - (float)dz;
+        // boundary neighbours (block 0): fluid a only (B<-B pairs are never evaluated, Eq. 36)
+        if (a_fluid) {
+          const uint32_t b0 = A.cellstart[lin2], b1 = A.cellstart[lin2 + 1];
+          for (uint32_t b = b0; b < b1; b++) {
+            const float4 pb = A.posu[b];
+            const float dux = ox - pb.x, duy = DIM == 3 ? oy - pb.y : 0.f, duz = oz - pb.z;
+            const float r2u = pair_r2u<DIM>(dux, duy, duz);
+            if (r2u < C.R2u) {
+              nb++;
+              const float4 vb = A.velp[b];
+              if (C.ddt_over_boundary)
+                pair_fluid<true>(C, dux, duy, duz, r2u, pa.w, inv_rho_a, va.w, va.x, va.y, va.z, pb, vb, S);
+              else
+                pair_fluid<false>(C, dux, duy, duz, r2u, pa.w, inv_rho_a, va.w, va.x, va.y, va.z, pb, vb, S);
+            }
+          }
+        }
+        // fluid neighbours (block 1)
+        {
+          const uint32_t b0 = A.cellstart[C.ncells + lin2], b1 = A.cellstart[C.ncells + lin2 + 1];
+          for (uint32_t b = b0; b < b1; b++) {
+            const float4 pb = A.posu[b];
+            const float dux = ox - pb.x, duy = DIM == 3 ? oy - pb.y : 0.f, duz = oz - pb.z;
+            const float r2u = pair_r2u<DIM>(dux, duy, duz);
+            if (r2u < C.R2u && b != a) {          // self excluded by index (A17)
+              nb++;
+              const float4 vb = A.velp[b];
+              if (a_fluid)
+                pair_fluid<true>(C, dux, duy, duz, r2u, pa.w, inv_rho_a, va.w, va.x, va.y, va.z, pb, vb, S);
+              else
+                pair_bound(C, dux, duy, duz, r2u, va.x, va.y, va.z, pb, vb, S);
+            }
+          }
+        }
+      }
+    }
+  }
+  const float4 out = finish_particle(C, a_fluid, pa.w, S);
+  A.acc[a] = out;
+  if (A.nbcount) A.nbcount[a] = nb;
+  if (a_fluid) f2 = fmaxf(f2, fmaf(out.x, out.x, fmaf(out.y, out.y, out.z * out.z)));
+  visc = fmaxf(visc, S.visc * C.c_mu);
+  nb_out += nb;
+}

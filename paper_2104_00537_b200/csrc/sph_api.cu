@@ -278,7 +278,10 @@ int run_pi(sph_ctx* ctx) {
   A.n = ctx->n;
   bool done = false;
   if (ctx->pi_kernel == 2) done = pi_tiled(ctx->C, A, s) == 0;
-  if (!done) pi_gather(ctx->C, A, s);
+  if (!done) {
+    pi_gather(ctx->C, A, s);
+    if (ctx->pi_kernel == 2) ctx->pi_kernel = 1;   // configuration not supported by the tiled kernel
+  }
   ctx->n_launch += 2;
   ctx->n_pi += 1;
   CK(cudaGetLastError());
@@ -320,7 +323,7 @@ SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
   ctx->key_bits = 0;
   for (uint32_t v = 2u * ctx->C.ncells; v; v >>= 1) ctx->key_bits++;
   if (ctx->key_bits == 0) ctx->key_bits = 1;
-  ctx->pi_kernel = params->pi_kernel == 0 ? 1 : params->pi_kernel;
+  ctx->pi_kernel = params->pi_kernel == 0 ? 2 : params->pi_kernel;   // auto: tiled, which falls back per call
   ctx->cellstart = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * ((size_t)ctx->nkeys + 1));
   ctx->sc = (DevScalars*)dalloc(ctx, sizeof(DevScalars));
   ctx->digit_total = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * 256 * 4);

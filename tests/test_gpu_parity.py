@@ -184,10 +184,11 @@ def test_all_boundary_and_out_of_grid(sph, pi_kernel):
 
 
 @pytest.mark.parametrize("pi_kernel", KERNELS)
-def test_crowded_cells_and_coincident_particles(sph, pi_kernel):
-    # 4000 particles in a 2.5-cell blob (hundreds per cell) + exact duplicates (r = 0, A17)
+@pytest.mark.parametrize("n", [4000, 7000])
+def test_crowded_cells_and_coincident_particles(sph, pi_kernel, n):
+    # n particles in a 2.5-cell blob (hundreds per cell) + exact duplicates (r = 0, A17); the larger case
+    # exceeds the tiled kernel's shared-memory staging capacity and takes its overflow path
     p = small_params()
-    n = 4000
     idx = np.arange(n)
     pos = 0.2 + 0.1 * np.stack([wl.uniform01(9, idx, k) for k in range(3)], 1)
     pos[100:120] = pos[200:220]                           # coincident distinct pairs
