@@ -63,7 +63,8 @@ typedef struct sph_params {
   int32_t cell_div;          /* k in {1,2,3}: cubic cells of size 2h/k, (2k+1)^dim-cell stencil.     */
                              /*   k=1: "cells of size 2h"; k=2: "size h" (635)        */
   double cell_size;          /* 0 -> 2h/k; else >= 2h/k, one value for all axes (C1)                 */
-  int32_t pi_kernel;         /* interaction kernel: 0 auto, 1 gather (thread/particle), 2 tiled smem */
+  int32_t pi_kernel;         /* interaction kernel: 0 auto, 1 gather (thread/particle), 2 tiled smem, */
+                             /*   3 quad (3-D, cell_div 1: conflict-free smem + packed FP32x2)       */
   int32_t count_neighbours;  /* 1: keep per-particle neighbour counts (SPH_NBCOUNT); costs a store   */
   sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
   sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */

@@ -1,0 +1,486 @@
+// Particle interaction (PI) task, "quad" kernel for sm_100a: 3-D, cells of size 2h (cell_div = 1).
+//
+// Same tile staging as pi_tiled.cu (a CTA owns 2x2x2 cells and stages them plus a one-cell halo in shared
+// memory with exact tile-centred coordinates, C1/C2), but the work of a warp is organised so that every
+// shared-memory access of the hot loops is bank-conflict free and the pair arithmetic runs on packed
+// FP32x2 instructions (FFMA2/FADD2/FMUL2, new on sm_100):
+//
+//   a-group : 8 particles a of one cell = 4 quarter-warps x 2.  Quarter-warp q owns the pair (a_2q, a_2q+1);
+//             its 8 lanes r = 0..7 own the candidates b whose staged index is congruent to r modulo 8.
+//   T phase : (test) lane (q, r) walks the candidate runs 16 candidates per step: one LDS.128 brings the
+//             half-precision test records of candidates 16g+r and 16g+r+8 (packed as half2), three HFMA2 and
+//             one HSET2 per a evaluate the expanded-form prefilter |b|^2 - 2 a.b < R^2 + margin - |a|^2 for
+//             both candidates at once.  The prefilter is conservative (margin > its rounding error);
+//             the bits of both a are OR-ed into one 32-bit word per 16 steps and stored per lane.
+//   P phase : (pair) each lane pops its own words.  Every popped b is loaded once (two LDS.128, conflict free
+//             because the 8 lanes of a quarter-warp hold 8 different residues) and evaluated against BOTH a of
+//             the lane with packed FP32x2 arithmetic, b entering as a broadcast scalar operand.  The exact
+//             canonical predicate C2 (fp32, individually rounded) decides membership; a b that is a neighbour
+//             of only one of the two a contributes exactly 0 to the other (the kernel weight is clamped at 0).
+//   reduce  : the partial sums of the 8 lanes of a quarter-warp are combined with 3 butterfly shuffles
+//             (fixed order, deterministic) and lane r = 0 writes the two results.
+//
+// What is kept from the paper: cell-linked list, particles sorted by cell, fp32 cell-relative positions
+// (PAPER.md:558, 572).  What differs: the thread-per-particle loop with a branch per candidate.
+#include <cuda_fp16.h>
+
+#include "pi_common.cuh"
+
+namespace {
+
+constexpr int QT = 2;                     // tile: QT^3 centre cells
+constexpr int QS = QT + 2;                // staged cells per axis
+constexpr int QNCELL = QS * QS * QS;      // 64 staged cells per type block
+constexpr int QNR = 2 * QNCELL;           // staged ranges: block 0 = boundary, block 1 = fluid
+constexpr int QNSEG = 2 * QT * QT * QT;   // a-segments: (block, centre cell)
+constexpr int QW = 10;                    // bitmap words per lane per round
+constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
+constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
+
+__device__ __forceinline__ int qrange(int blk, int ix, int iy, int iz) {   // staged indices, 0-based
+  return ((blk * QS + iz) * QS + iy) * QS + ix;
+}
+
+struct QSmem {
+  float4* rpos;       // (x, y, z, rho): exact tile-centred coordinates + density
+  float4* rvel;       // (vx, vy, vz, P)
+  uint4* tst;         // half2-packed test records: entry g*8 + r = candidates 16g+r (low halves) and 16g+r+8
+  uint32_t* bm;       // [warp][QW][32] bitmap words
+  uint32_t* desc;     // [warp][QW] first candidate index of the word | ddt flag << 31
+  uint32_t* soff;     // QNR + 1
+  uint32_t* gstart;   // QNR
+  uint32_t* seg;      // [0] group counter, [1..QNSEG+1] a-group prefix
+};
+
+__device__ __forceinline__ uint32_t h2_as_u32(__half2 h) { return *reinterpret_cast<uint32_t*>(&h); }
+__device__ __forceinline__ __half2 u32_as_h2(uint32_t u) { return *reinterpret_cast<__half2*>(&u); }
+
+// Packed state of the two particles a of a lane.
+struct PairA {
+  float2 x, y, z, vx, vy, vz, rho, inv_rho, P;
+};
+struct PairAcc2 {
+  float2 sx, sy, sz, sc, sd;
+  float visc0, visc1;
+  unsigned nb0, nb1;
+};
+
+__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
+
+// One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free.  A b outside the
+// support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record) gets weight 0:
+// w = max(1 - q/2, 0).  nb counts the exact canonical predicate C2.
+template <bool A_FLUID>
+__device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const float4 pb, const float4 vb,
+                                      float ddtw, PairAcc2& A) {
+  const float2 dux = __fadd2_rn(a.x, bc(-pb.x));   // exact (C1)
+  const float2 duy = __fadd2_rn(a.y, bc(-pb.y));
+  const float2 duz = __fadd2_rn(a.z, bc(-pb.z));
+  float2 r2 = __fmul2_rn(dux, dux);                // C2: individually rounded
+  r2 = __ffma2_rn(duy, duy, r2);
+  r2 = __ffma2_rn(duz, duz, r2);
+  A.nb0 += r2.x < C.R2u ? 1u : 0u;
+  A.nb1 += r2.y < C.R2u ? 1u : 0u;
+  const float2 s = make_float2(fast_sqrt(r2.x), fast_sqrt(r2.y));
+  float2 w = __ffma2_rn(s, bc(-C.qscale), bc(1.0f));           // 1 - q/2   (Eq. 11)
+  w.x = fmaxf(w.x, 0.f);
+  w.y = fmaxf(w.y, 0.f);
+  const float2 w3 = __fmul2_rn(__fmul2_rn(w, w), w);           // grad_a W_ab = Cf w^3 cs du
+  const float inv_rho_b = fast_rcp(pb.w);
+  const float2 dvx = __fadd2_rn(a.vx, bc(-vb.x));
+  const float2 dvy = __fadd2_rn(a.vy, bc(-vb.y));
+  const float2 dvz = __fadd2_rn(a.vz, bc(-vb.z));
+  float2 dot = __fmul2_rn(dvx, dux);                           // v_ab . r_ab / cs
+  dot = __ffma2_rn(dvy, duy, dot);
+  dot = __ffma2_rn(dvz, duz, dot);
+  const float2 gb = __fmul2_rn(w3, bc(inv_rho_b));
+  A.sc = __ffma2_rn(gb, dot, A.sc);
+  if (A_FLUID) {
+    const float2 drho = __fadd2_rn(a.rho, bc(-pb.w));
+    A.sd = __ffma2_rn(__fmul2_rn(gb, bc(ddtw)), drho, A.sd);
+    const float2 rs = __fadd2_rn(a.rho, bc(pb.w));
+    const float2 den = __fmul2_rn(__fadd2_rn(r2, bc(C.eta2u)), rs);
+    const float2 x = make_float2(fast_rcp(den.x), fast_rcp(den.y));
+    const float2 mu = __fmul2_rn(dot, __fmul2_rn(x, rs));      // mu_ab / c_mu   (Eq. 21, A12)
+    A.visc0 = fmaxf(A.visc0, fabsf(mu.x));
+    A.visc1 = fmaxf(A.visc1, fabsf(mu.y));
+    const float2 t = __fmul2_rn(make_float2(fminf(dot.x, 0.f), fminf(dot.y, 0.f)), x);   // approaching pairs only
+    const float2 pp = __fmul2_rn(__fadd2_rn(a.P, bc(vb.w)), __fmul2_rn(a.inv_rho, bc(inv_rho_b)));
+    const float2 coef = __fmul2_rn(w3, __ffma2_rn(bc(C.c_pi), t, pp));
+    A.sx = __ffma2_rn(coef, dux, A.sx);
+    A.sy = __ffma2_rn(coef, duy, A.sy);
+    A.sz = __ffma2_rn(coef, duz, A.sz);
+  }
+}
+
+// Sum over the 8 lanes of a quarter-warp (butterfly, fixed order).
+__device__ __forceinline__ float qsum(float v) {
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  v += __shfl_xor_sync(0xffffffffu, v, 2);
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  return v;
+}
+__device__ __forceinline__ float qmax(float v) {
+  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
+  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
+  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 4));
+  return v;
+}
+__device__ __forceinline__ unsigned qsumu(unsigned v) {
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  v += __shfl_xor_sync(0xffffffffu, v, 2);
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  return v;
+}
+
+// One a-group: up to 8 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
+// A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw / descw are this warp's bitmap and descriptor areas.
+template <bool A_FLUID>
+__device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint32_t* bmw,
+                                              uint32_t* descw, int cx, int cy, int cz, unsigned cell_start,
+                                              unsigned n_a, unsigned grp, unsigned total, float& f2max,
+                                              float& viscmax, unsigned int& nbsum) {
+  const int lane = threadIdx.x & 31, q = lane >> 3, r = lane & 7;
+  const unsigned t0 = grp * 8 + 2 * q, t1 = t0 + 1;
+  const bool act0 = t0 < n_a, act1 = t1 < n_a;
+  const unsigned ja0 = cell_start + (act0 ? t0 : 0), ja1 = cell_start + (act1 ? t1 : 0);
+
+  // ---- state of the two a of this lane (inactive: far away, never accepted) ----
+  PairA a;
+  __half2 nx0, ny0, nz0, th0, nx1, ny1, nz1, th1;
+  {
+    float4 p0 = S.rpos[ja0], v0 = S.rvel[ja0], p1 = S.rpos[ja1], v1 = S.rvel[ja1];
+    if (!act0) { p0 = make_float4(-Q_FAR, -Q_FAR, -Q_FAR, 1.f); v0 = make_float4(0.f, 0.f, 0.f, 0.f); }
+    if (!act1) { p1 = make_float4(-Q_FAR, -Q_FAR, -Q_FAR, 1.f); v1 = make_float4(0.f, 0.f, 0.f, 0.f); }
+    a.x = make_float2(p0.x, p1.x); a.y = make_float2(p0.y, p1.y); a.z = make_float2(p0.z, p1.z);
+    a.rho = make_float2(p0.w, p1.w);
+    a.inv_rho = make_float2(fast_rcp(p0.w), fast_rcp(p1.w));
+    a.vx = make_float2(v0.x, v1.x); a.vy = make_float2(v0.y, v1.y); a.vz = make_float2(v0.z, v1.z);
+    a.P = make_float2(v0.w, v1.w);
+    // prefilter operands (half precision): s = |b|^2 - 2 a.b  <  thr = R2u + margin - |a|^2
+    const float thr0 = act0 ? (C.R2u + Q_MARGIN) - fmaf(p0.z, p0.z, fmaf(p0.y, p0.y, p0.x * p0.x)) : -60000.f;
+    const float thr1 = act1 ? (C.R2u + Q_MARGIN) - fmaf(p1.z, p1.z, fmaf(p1.y, p1.y, p1.x * p1.x)) : -60000.f;
+    nx0 = __float2half2_rn(act0 ? -2.f * p0.x : 0.f); ny0 = __float2half2_rn(act0 ? -2.f * p0.y : 0.f);
+    nz0 = __float2half2_rn(act0 ? -2.f * p0.z : 0.f); th0 = __half2half2(__float2half_ru(thr0));
+    nx1 = __float2half2_rn(act1 ? -2.f * p1.x : 0.f); ny1 = __float2half2_rn(act1 ? -2.f * p1.y : 0.f);
+    nz1 = __float2half2_rn(act1 ? -2.f * p1.z : 0.f); th1 = __half2half2(__float2half_ru(thr1));
+  }
+  PairAcc2 acc;
+  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = make_float2(0.f, 0.f);
+  acc.visc0 = acc.visc1 = 0.f;
+  acc.nb0 = acc.nb1 = 0u;
+
+  const float ddtb = C.ddt_over_boundary ? 1.f : 0.f;
+  const int nruns = A_FLUID ? 18 : 9;      // fluid a: 9 boundary-block rows then 9 fluid rows; boundary a: fluid rows
+  int ri = 0;
+  int gw = -1, g_first = 0, g_last = -1;
+  unsigned j0 = 0, j1 = 0;
+  bool run_ddt = true;
+
+  while (true) {
+    // ================= T phase: fill up to QW words =================
+    int nw = 0;
+    unsigned cnt = 0;
+    while (nw < QW && ri < nruns) {
+      if (gw < 0) {   // open run ri
+        const int blk_b = A_FLUID ? (ri >= 9 ? 1 : 0) : 1;
+        const int k = ri % 9, iz = 1 + cz + (k / 3 - 1), iy = 1 + cy + (k % 3 - 1);
+        j0 = S.soff[qrange(blk_b, cx, iy, iz)];
+        j1 = S.soff[qrange(blk_b, cx + 2, iy, iz) + 1];
+        if (j1 <= j0) { ri++; continue; }
+        g_first = (int)(j0 >> 4);
+        g_last = (int)((j1 - 1) >> 4);
+        gw = g_first;
+        run_ddt = blk_b == 1 || C.ddt_over_boundary != 0;
+      }
+      const int nstep = min(16, g_last - gw + 1);
+      const uint4* tp = S.tst + gw * 8 + r;
+      unsigned u = 0;
+#pragma unroll
+      for (int i = 0; i < 16; i++) {
+        if (i < nstep) {
+          const uint4 t = tp[i * 8];
+          const __half2 bx = u32_as_h2(t.x), by = u32_as_h2(t.y), bz = u32_as_h2(t.z), bw = u32_as_h2(t.w);
+          const __half2 s0 = __hfma2(nz0, bz, __hfma2(ny0, by, __hfma2(nx0, bx, bw)));
+          const __half2 s1 = __hfma2(nz1, bz, __hfma2(ny1, by, __hfma2(nx1, bx, bw)));
+          const unsigned m = __hlt2_mask(s0, th0) | __hlt2_mask(s1, th1);
+          u |= m & (0x00010001u << i);
+        }
+      }
+      // candidates of the first / last group that lie outside the run [j0, j1)
+      unsigned kill = 0;
+      if (gw == g_first) {
+        const unsigned c = (unsigned)gw * 16u + (unsigned)r;
+        if (c < j0) kill |= 1u;
+        if (c + 8u < j0) kill |= 0x10000u;
+      }
+      if (g_last - gw < 16) {
+        const unsigned c = (unsigned)g_last * 16u + (unsigned)r;
+        const int il = g_last - gw;
+        if (c >= j1) kill |= 1u << il;
+        if (c + 8u >= j1) kill |= 0x10000u << il;
+      }
+      u &= ~kill;
+      bmw[nw * 32 + lane] = u;
+      if (lane == 0) descw[nw] = ((unsigned)gw * 16u) | (run_ddt ? 0x80000000u : 0u);
+      cnt += (u != 0u) ? (unsigned)__popc(u) : 1u;   // a zero word costs one idle iteration
+      nw++;
+      gw += 16;
+      if (gw > g_last) { ri++; gw = -1; }
+    }
+    if (nw == 0) break;
+    __syncwarp();
+
+    // ================= P phase: every lane pops its own words =================
+    const unsigned n_it = __reduce_max_sync(0xffffffffu, cnt);
+    unsigned cur = 0, base_r = 0;
+    int wi = 0;
+    float ddtw = 0.f;
+#pragma unroll 2
+    for (unsigned it = 0; it < n_it; it++) {
+      if (cur == 0u && wi < nw) {
+        cur = bmw[wi * 32 + lane];
+        const unsigned d = descw[wi];
+        base_r = (d & 0x7fffffffu) + (unsigned)r;
+        ddtw = (d >> 31) ? 1.f : ddtb;
+        wi++;
+      }
+      const int p = __ffs(cur) - 1;
+      const unsigned idx = cur != 0u ? base_r + (((unsigned)p & 15u) << 4) + (((unsigned)p >> 4) << 3) : total;
+      cur &= cur - 1u;
+      const float4 pb = S.rpos[idx];
+      const float4 vb = S.rvel[idx];
+      pair2<A_FLUID>(C, a, pb, vb, ddtw, acc);
+    }
+    __syncwarp();
+    if (ri >= nruns) break;
+  }
+
+  // ---- combine the 8 lanes of each quarter-warp; lane r = 0 writes both particles ----
+  acc.sc.x = qsum(acc.sc.x); acc.sc.y = qsum(acc.sc.y);
+  acc.nb0 = qsumu(acc.nb0); acc.nb1 = qsumu(acc.nb1);
+  if (A_FLUID) {
+    acc.sx.x = qsum(acc.sx.x); acc.sx.y = qsum(acc.sx.y);
+    acc.sy.x = qsum(acc.sy.x); acc.sy.y = qsum(acc.sy.y);
+    acc.sz.x = qsum(acc.sz.x); acc.sz.y = qsum(acc.sz.y);
+    acc.sd.x = qsum(acc.sd.x); acc.sd.y = qsum(acc.sd.y);
+    acc.visc0 = qmax(acc.visc0); acc.visc1 = qmax(acc.visc1);
+  }
+  if (r == 0) {
+    const int ra = qrange(A_FLUID ? 1 : 0, 1 + cx, 1 + cy, 1 + cz);
+    const unsigned gbase = S.gstart[ra] - S.soff[ra];
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+      if (h == 0 ? act0 : act1) {
+        PairAcc pa1;
+        pa1.sx = h ? acc.sx.y : acc.sx.x; pa1.sy = h ? acc.sy.y : acc.sy.x; pa1.sz = h ? acc.sz.y : acc.sz.x;
+        pa1.sc = h ? acc.sc.y : acc.sc.x; pa1.sd = h ? acc.sd.y : acc.sd.x;
+        pa1.visc = h ? acc.visc1 : acc.visc0;
+        unsigned nb = h ? acc.nb1 : acc.nb0;
+        if (A_FLUID) nb -= 1u;   // the particle itself passed the test at r = 0 and contributed exactly 0 (A17)
+        const unsigned ga = gbase + (h ? ja1 : ja0);
+        const float4 out = finish_particle(C, A_FLUID, h ? a.rho.y : a.rho.x, pa1);
+        A.acc[ga] = out;
+        if (A.nbcount) A.nbcount[ga] = nb;
+        if (A_FLUID) f2max = fmaxf(f2max, fmaf(out.x, out.x, fmaf(out.y, out.y, out.z * out.z)));
+        viscmax = fmaxf(viscmax, pa1.visc * C.c_mu);
+        nbsum += nb;
+      }
+    }
+  }
+}
+
+template <int NT, int NMAX>
+__global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int ntx, int nty) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int NWARP = NT / 32;
+  QSmem S;
+  S.rpos = reinterpret_cast<float4*>(smem_raw);
+  S.rvel = S.rpos + NMAX;
+  S.tst = reinterpret_cast<uint4*>(S.rvel + NMAX);
+  S.bm = reinterpret_cast<uint32_t*>(S.tst + (NMAX / 16) * 8);
+  S.desc = S.bm + NWARP * QW * 32;
+  S.soff = S.desc + NWARP * QW;
+  S.gstart = S.soff + (QNR + 1);
+  S.seg = S.gstart + QNR;
+  __shared__ uint32_t s_cnt[QNR];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tx = blockIdx.x % ntx, ty = (blockIdx.x / ntx) % nty, tz = blockIdx.x / (ntx * nty);
+  const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
+
+  // 1. global ranges of the staged cells (both type blocks)
+  for (int rr = tid; rr < QNR; rr += NT) {
+    const int blk = rr / QNCELL, c = rr % QNCELL;
+    const int ix = c % QS, iy = (c / QS) % QS, iz = c / (QS * QS);
+    int g[3] = {ox + ix - 1, oy + iy - 1, oz + iz - 1};
+    bool valid = true;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+      if (C.per[k]) g[k] = (g[k] + C.nc[k]) % C.nc[k];
+      else if (g[k] < 0 || g[k] >= C.nc[k]) valid = false;
+    }
+    uint32_t g0 = 0, n = 0;
+    if (valid) {
+      const uint32_t key = (uint32_t)blk * C.ncells + (uint32_t)g[0] +
+                           (uint32_t)C.nc[0] * ((uint32_t)g[1] + (uint32_t)C.nc[1] * (uint32_t)g[2]);
+      g0 = A.cellstart[key];
+      n = A.cellstart[key + 1] - g0;
+    }
+    s_cnt[rr] = n;
+    S.gstart[rr] = g0;
+  }
+  __syncthreads();
+  if (warp == 0) {   // exclusive scan of the QNR counts
+    constexpr int PER = (QNR + 31) / 32;
+    uint32_t v[PER], sum = 0;
+#pragma unroll
+    for (int i = 0; i < PER; i++) {
+      const int rr = lane * PER + i;
+      v[i] = rr < QNR ? s_cnt[rr] : 0u;
+      sum += v[i];
+    }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += up;
+    }
+    uint32_t run = inc - sum;
+#pragma unroll
+    for (int i = 0; i < PER; i++) {
+      const int rr = lane * PER + i;
+      if (rr < QNR) S.soff[rr] = run;
+      run += v[i];
+    }
+    if (lane == 31) S.soff[QNR] = inc;
+  }
+  __syncthreads();
+
+  // a-segments (block, centre cell) and the a-group prefix for dynamic scheduling
+  const int vx = min(QT, C.nc[0] - ox), vy = min(QT, C.nc[1] - oy), vz = min(QT, C.nc[2] - oz);
+  if (tid == 0) {
+    uint32_t run = 0;
+    for (int s = 0; s < QNSEG; s++) {
+      const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
+      uint32_t n = 0;
+      if (cx < vx && cy < vy && cz < vz) n = s_cnt[qrange(blk, 1 + cx, 1 + cy, 1 + cz)];
+      S.seg[1 + s] = run;
+      run += (n + 7) / 8;
+    }
+    S.seg[1 + QNSEG] = run;
+    S.seg[0] = 0;
+  }
+  __syncthreads();
+  const uint32_t ngroups = S.seg[1 + QNSEG];
+  if (ngroups == 0) return;                       // nothing to compute in this tile (air)
+  const uint32_t total = S.soff[QNR];
+
+  float f2max = 0.f, viscmax = 0.f;
+  unsigned int nbsum = 0;
+
+  if (total + 1 > (uint32_t)NMAX) {
+    // staged set does not fit in shared memory (very crowded cells): per-particle global gather
+    for (int s = 0; s < QNSEG; s++) {
+      const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
+      if (cx >= vx || cy >= vy || cz >= vz) continue;
+      const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
+      const uint32_t g0 = S.gstart[rr], len = s_cnt[rr];
+      for (uint32_t i = tid; i < len; i += NT) gather_one<3>(C, A, g0 + i, blk == 1, f2max, viscmax, nbsum);
+    }
+    reduce_scalars(A.sc, f2max, viscmax, nbsum);
+    return;
+  }
+
+  // 2. stage particles with tile-centred coordinates: u + integer cell offset - QT/2.  Exact: every value is a
+  //    multiple of 2^-22 with magnitude <= 2, so all differences are exact in fp32 (C1/C2).
+  for (int rr = warp; rr < QNR; rr += NWARP) {
+    const uint32_t n = s_cnt[rr];
+    if (n == 0) continue;
+    const int c = rr % QNCELL;
+    const float fx = (float)(c % QS - 1) - 0.5f * QT, fy = (float)((c / QS) % QS - 1) - 0.5f * QT,
+                fz = (float)(c / (QS * QS) - 1) - 0.5f * QT;
+    const uint32_t g0 = S.gstart[rr], d0 = S.soff[rr];
+    for (uint32_t i = lane; i < n; i += 32) {
+      const float4 p = A.posu[g0 + i];
+      const float4 v = A.velp[g0 + i];
+      S.rpos[d0 + i] = make_float4(p.x + fx, p.y + fy, p.z + fz, p.w);
+      S.rvel[d0 + i] = v;
+    }
+  }
+  if (tid == 0) {   // dummy record: popped by lanes that have run out of work, never within any support
+    S.rpos[total] = make_float4(Q_FAR, Q_FAR, Q_FAR, 1.0f);
+    S.rvel[total] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  __syncthreads();
+  // 3. half-precision test records, two candidates per half2: entry g*8 + r <- candidates 16g + r, 16g + r + 8
+  {
+    const uint32_t nent = ((total + 15) / 16) * 8;
+    for (uint32_t e = tid; e < nent; e += NT) {
+      const uint32_t c0 = (e >> 3) * 16 + (e & 7), c1 = c0 + 8;
+      float4 p0 = make_float4(0.f, 0.f, 0.f, 0.f), p1 = p0;
+      if (c0 < total) p0 = S.rpos[c0];
+      if (c1 < total) p1 = S.rpos[c1];
+      const __half2 hx = __floats2half2_rn(p0.x, p1.x), hy = __floats2half2_rn(p0.y, p1.y),
+                    hz = __floats2half2_rn(p0.z, p1.z);
+      const float2 fx = __half22float2(hx), fy = __half22float2(hy), fz = __half22float2(hz);
+      float w0 = fmaf(fz.x, fz.x, fmaf(fy.x, fy.x, fx.x * fx.x));   // |b|^2 of the rounded coordinates
+      float w1 = fmaf(fz.y, fz.y, fmaf(fy.y, fy.y, fx.y * fx.y));
+      if (c0 >= total) w0 = 60000.f;                                 // padding: never accepted
+      if (c1 >= total) w1 = 60000.f;
+      const __half2 hw = __floats2half2_rn(w0, w1);
+      S.tst[e] = make_uint4(h2_as_u32(hx), h2_as_u32(hy), h2_as_u32(hz), h2_as_u32(hw));
+    }
+  }
+  __syncthreads();
+
+  // 4. a-groups, taken dynamically by the warps
+  uint32_t* bmw = S.bm + warp * QW * 32;
+  uint32_t* descw = S.desc + warp * QW;
+  while (true) {
+    uint32_t gi = 0;
+    if (lane == 0) gi = atomicAdd(&S.seg[0], 1u);
+    gi = __shfl_sync(0xffffffffu, gi, 0);
+    if (gi >= ngroups) break;
+    int s = 0;
+    while (s + 1 < QNSEG && gi >= S.seg[1 + s + 1]) s++;
+    const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
+    const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
+    const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
+    if (blk == 1) process_group<true>(C, A, S, bmw, descw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    else process_group<false>(C, A, S, bmw, descw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+  }
+  reduce_scalars(A.sc, f2max, viscmax, nbsum);
+}
+
+template <int NT, int NMAX>
+int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
+  const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
+  constexpr int NWARP = NT / 32;
+  const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint4) * (NMAX / 16) * 8 +
+                      sizeof(uint32_t) * (NWARP * QW * 32 + NWARP * QW + (QNR + 1) + QNR + (QNSEG + 2));
+  static bool configured = false;
+  if (!configured) {
+    if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+        cudaSuccess) {
+      cudaGetLastError();
+      return -1;
+    }
+    configured = true;
+  }
+  const long long ntiles = (long long)ntx * nty * ntz;
+  if (ntiles > 0x7fffffffLL) return -1;
+  k_pi_quad<NT, NMAX><<<(unsigned)ntiles, NT, smem, s>>>(C, A, ntx, nty);
+  return 0;
+}
+
+}  // namespace
+
+// Returns 0 if the quad kernel was launched, -1 if this configuration is not supported (caller falls back to
+// the tiled kernel): 3-D, cells of size 2h (27-cell stencil), eta^2 > 0.
+int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
+  if (A.n == 0) return 0;
+  if (C.dim != 3 || C.k != 1) return -1;
+  if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
+  return launch_quad<384, 4992>(C, A, s);
+}

@@ -153,7 +153,7 @@ int validate(const sph_params* p, std::string& why) {
   if (!(p->cfl > 0)) return bad("cfl must be positive");
   if (p->alpha < 0 || p->delta < 0 || p->eta2_coef < 0) return bad("alpha, delta, eta2_coef must be >= 0");
   if (p->cell_div < 1 || p->cell_div > 3) return bad("cell_div must be 1, 2 or 3");
-  if (p->pi_kernel < 0 || p->pi_kernel > 2) return bad("pi_kernel must be 0, 1 or 2");
+  if (p->pi_kernel < 0 || p->pi_kernel > 3) return bad("pi_kernel must be 0, 1, 2 or 3");
   const double cs_min = 2.0 * p->h / p->cell_div;
   if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
   for (int k = 0; k < 3; k++) {
@@ -277,7 +277,11 @@ int run_pi(sph_ctx* ctx) {
   A.sc = ctx->sc;
   A.n = ctx->n;
   bool done = false;
-  if (ctx->pi_kernel == 2) done = pi_tiled(ctx->C, A, s) == 0;
+  if (ctx->pi_kernel == 3) {
+    done = pi_quad(ctx->C, A, s) == 0;
+    if (!done) ctx->pi_kernel = 2;                 // configuration not supported by the quad kernel
+  }
+  if (!done && ctx->pi_kernel == 2) done = pi_tiled(ctx->C, A, s) == 0;
   if (!done) {
     pi_gather(ctx->C, A, s);
     if (ctx->pi_kernel == 2) ctx->pi_kernel = 1;   // configuration not supported by the tiled kernel
@@ -323,7 +327,7 @@ SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
   ctx->key_bits = 0;
   for (uint32_t v = 2u * ctx->C.ncells; v; v >>= 1) ctx->key_bits++;
   if (ctx->key_bits == 0) ctx->key_bits = 1;
-  ctx->pi_kernel = params->pi_kernel == 0 ? 2 : params->pi_kernel;   // auto: tiled, which falls back per call
+  ctx->pi_kernel = params->pi_kernel == 0 ? 3 : params->pi_kernel;   // auto: quad -> tiled -> gather, falling back per call
   ctx->cellstart = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * ((size_t)ctx->nkeys + 1));
   ctx->sc = (DevScalars*)dalloc(ctx, sizeof(DevScalars));
   ctx->digit_total = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * 256 * 4);

@@ -86,6 +86,7 @@ struct PiArgs {
 };
 void pi_gather(const DevConsts& C, const PiArgs& A, cudaStream_t s);
 int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s);   // returns 0, or -1 if unsupported config
+int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s);    // 3-D, cell_div 1 only; 0 or -1 likewise
 void pi_reset_scalars(DevScalars* sc, cudaStream_t s);
 
 // ---- system update (su_kernels.cu) ----
