@@ -33,7 +33,7 @@ constexpr int QS = QT + 2;                // staged cells per axis
 constexpr int QNCELL = QS * QS * QS;      // 64 staged cells per type block
 constexpr int QNR = 2 * QNCELL;           // staged ranges: block 0 = boundary, block 1 = fluid
 constexpr int QNSEG = 2 * QT * QT * QT;   // a-segments: (block, centre cell)
-constexpr int QW = 10;                    // bitmap words per lane per round
+constexpr int QW = 9;                     // bitmap words per lane per round
 constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
 constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
 
@@ -45,8 +45,7 @@ struct QSmem {
   float4* rpos;       // (x, y, z, rho): exact tile-centred coordinates + density
   float4* rvel;       // (vx, vy, vz, P)
   uint4* tst;         // half2-packed test records: entry g*8 + r = candidates 16g+r (low halves) and 16g+r+8
-  uint32_t* bm;       // [warp][QW][32] bitmap words
-  uint32_t* desc;     // [warp][QW] first candidate index of the word | ddt flag << 31
+  uint2* bm;          // [warp][QW][32] (bitmap word, byte address of the record of its bit 0)
   uint32_t* soff;     // QNR + 1
   uint32_t* gstart;   // QNR
   uint32_t* seg;      // [0] group counter, [1..QNSEG+1] a-group prefix
@@ -55,17 +54,59 @@ struct QSmem {
 __device__ __forceinline__ uint32_t h2_as_u32(__half2 h) { return *reinterpret_cast<uint32_t*>(&h); }
 __device__ __forceinline__ __half2 u32_as_h2(uint32_t u) { return *reinterpret_cast<__half2*>(&u); }
 
+// Packed FP32x2 values live in 64-bit registers (an aligned register pair), so that ptxas keeps the two halves
+// together and needs no moves around FADD2 / FMUL2 / FFMA2.  A scalar operand is written as the pair {s, s};
+// ptxas folds it into the instruction's scalar-broadcast operand form.
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 f2_pack(float lo, float hi) {
+  f2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ f2 f2_bc(float s) { return f2_pack(s, s); }
+// Pack two scalars through a packed add of +0 (exact up to the sign of zero), so that the result is born in an aligned register pair
+// and stays there (a plain mov.b64 is re-materialised by ptxas with two moves at every use).
+__device__ __forceinline__ f2 f2_pack_pinned(float lo, float hi) {
+  f2 r;
+  asm volatile("{.reg .b64 t, o; mov.b64 t, {%1, %2}; mov.b64 o, {%3, %3}; add.rn.f32x2 %0, t, o;}"
+               : "=l"(r) : "f"(lo), "f"(hi), "f"(0.0f));
+  return r;
+}
+__device__ __forceinline__ float f2_lo(f2 v) {
+  float lo, hi;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  return lo;
+}
+__device__ __forceinline__ float f2_hi(f2 v) {
+  float lo, hi;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  return hi;
+}
+__device__ __forceinline__ f2 f2_add(f2 a, f2 b) {
+  f2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f2 f2_mul(f2 a, f2 b) {
+  f2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
+  f2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+
 // Packed state of the two particles a of a lane.
 struct PairA {
-  float2 x, y, z, vx, vy, vz, rho, inv_rho, P;
+  f2 x, y, z, vx, vy, vz, rho, inv_rho, P;
 };
 struct PairAcc2 {
-  float2 sx, sy, sz, sc, sd;
+  f2 sx, sy, sz, sc, sd;
   float visc0, visc1;
   unsigned nb0, nb1;
 };
-
-__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
 
 // One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free.  A b outside the
 // support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record) gets weight 0:
@@ -73,43 +114,42 @@ __device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }
 template <bool A_FLUID>
 __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const float4 pb, const float4 vb,
                                       float ddtw, PairAcc2& A) {
-  const float2 dux = __fadd2_rn(a.x, bc(-pb.x));   // exact (C1)
-  const float2 duy = __fadd2_rn(a.y, bc(-pb.y));
-  const float2 duz = __fadd2_rn(a.z, bc(-pb.z));
-  float2 r2 = __fmul2_rn(dux, dux);                // C2: individually rounded
-  r2 = __ffma2_rn(duy, duy, r2);
-  r2 = __ffma2_rn(duz, duz, r2);
-  A.nb0 += r2.x < C.R2u ? 1u : 0u;
-  A.nb1 += r2.y < C.R2u ? 1u : 0u;
-  const float2 s = make_float2(fast_sqrt(r2.x), fast_sqrt(r2.y));
-  float2 w = __ffma2_rn(s, bc(-C.qscale), bc(1.0f));           // 1 - q/2   (Eq. 11)
-  w.x = fmaxf(w.x, 0.f);
-  w.y = fmaxf(w.y, 0.f);
-  const float2 w3 = __fmul2_rn(__fmul2_rn(w, w), w);           // grad_a W_ab = Cf w^3 cs du
+  const f2 dux = f2_add(a.x, f2_bc(-pb.x));   // exact (C1)
+  const f2 duy = f2_add(a.y, f2_bc(-pb.y));
+  const f2 duz = f2_add(a.z, f2_bc(-pb.z));
+  f2 r2 = f2_mul(dux, dux);                   // C2: individually rounded
+  r2 = f2_fma(duy, duy, r2);
+  r2 = f2_fma(duz, duz, r2);
+  const float r2a = f2_lo(r2), r2b = f2_hi(r2);
+  A.nb0 += r2a < C.R2u ? 1u : 0u;
+  A.nb1 += r2b < C.R2u ? 1u : 0u;
+  f2 w = f2_fma(f2_pack(fast_sqrt(r2a), fast_sqrt(r2b)), f2_bc(-C.qscale), f2_bc(1.0f));   // 1 - q/2   (Eq. 11)
+  w = f2_pack(fmaxf(f2_lo(w), 0.f), fmaxf(f2_hi(w), 0.f));
+  const f2 w3 = f2_mul(f2_mul(w, w), w);      // grad_a W_ab = Cf w^3 cs du
   const float inv_rho_b = fast_rcp(pb.w);
-  const float2 dvx = __fadd2_rn(a.vx, bc(-vb.x));
-  const float2 dvy = __fadd2_rn(a.vy, bc(-vb.y));
-  const float2 dvz = __fadd2_rn(a.vz, bc(-vb.z));
-  float2 dot = __fmul2_rn(dvx, dux);                           // v_ab . r_ab / cs
-  dot = __ffma2_rn(dvy, duy, dot);
-  dot = __ffma2_rn(dvz, duz, dot);
-  const float2 gb = __fmul2_rn(w3, bc(inv_rho_b));
-  A.sc = __ffma2_rn(gb, dot, A.sc);
+  const f2 dvx = f2_add(a.vx, f2_bc(-vb.x));
+  const f2 dvy = f2_add(a.vy, f2_bc(-vb.y));
+  const f2 dvz = f2_add(a.vz, f2_bc(-vb.z));
+  f2 dot = f2_mul(dvx, dux);                  // v_ab . r_ab / cs
+  dot = f2_fma(dvy, duy, dot);
+  dot = f2_fma(dvz, duz, dot);
+  const f2 gb = f2_mul(w3, f2_bc(inv_rho_b));
+  A.sc = f2_fma(gb, dot, A.sc);
   if (A_FLUID) {
-    const float2 drho = __fadd2_rn(a.rho, bc(-pb.w));
-    A.sd = __ffma2_rn(__fmul2_rn(gb, bc(ddtw)), drho, A.sd);
-    const float2 rs = __fadd2_rn(a.rho, bc(pb.w));
-    const float2 den = __fmul2_rn(__fadd2_rn(r2, bc(C.eta2u)), rs);
-    const float2 x = make_float2(fast_rcp(den.x), fast_rcp(den.y));
-    const float2 mu = __fmul2_rn(dot, __fmul2_rn(x, rs));      // mu_ab / c_mu   (Eq. 21, A12)
-    A.visc0 = fmaxf(A.visc0, fabsf(mu.x));
-    A.visc1 = fmaxf(A.visc1, fabsf(mu.y));
-    const float2 t = __fmul2_rn(make_float2(fminf(dot.x, 0.f), fminf(dot.y, 0.f)), x);   // approaching pairs only
-    const float2 pp = __fmul2_rn(__fadd2_rn(a.P, bc(vb.w)), __fmul2_rn(a.inv_rho, bc(inv_rho_b)));
-    const float2 coef = __fmul2_rn(w3, __ffma2_rn(bc(C.c_pi), t, pp));
-    A.sx = __ffma2_rn(coef, dux, A.sx);
-    A.sy = __ffma2_rn(coef, duy, A.sy);
-    A.sz = __ffma2_rn(coef, duz, A.sz);
+    const f2 drho = f2_add(a.rho, f2_bc(-pb.w));
+    A.sd = f2_fma(f2_mul(gb, f2_bc(ddtw)), drho, A.sd);
+    const f2 rs = f2_add(a.rho, f2_bc(pb.w));
+    const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), rs);
+    const f2 x = f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den)));
+    const f2 mu = f2_mul(dot, f2_mul(x, rs));             // mu_ab / c_mu   (Eq. 21, A12)
+    A.visc0 = fmaxf(A.visc0, fabsf(f2_lo(mu)));
+    A.visc1 = fmaxf(A.visc1, fabsf(f2_hi(mu)));
+    const f2 t = f2_mul(f2_pack(fminf(f2_lo(dot), 0.f), fminf(f2_hi(dot), 0.f)), x);   // approaching pairs only
+    const f2 pp = f2_mul(f2_add(a.P, f2_bc(vb.w)), f2_mul(a.inv_rho, f2_bc(inv_rho_b)));
+    const f2 coef = f2_mul(w3, f2_fma(f2_bc(C.c_pi), t, pp));
+    A.sx = f2_fma(coef, dux, A.sx);
+    A.sy = f2_fma(coef, duy, A.sy);
+    A.sz = f2_fma(coef, duz, A.sz);
   }
 }
 
@@ -134,12 +174,11 @@ __device__ __forceinline__ unsigned qsumu(unsigned v) {
 }
 
 // One a-group: up to 8 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
-// A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw / descw are this warp's bitmap and descriptor areas.
+// A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw is this warp's bitmap area ([QW][32] uint2).
 template <bool A_FLUID>
-__device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint32_t* bmw,
-                                              uint32_t* descw, int cx, int cy, int cz, unsigned cell_start,
-                                              unsigned n_a, unsigned grp, unsigned total, float& f2max,
-                                              float& viscmax, unsigned int& nbsum) {
+__device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint2* bmw, int cx,
+                                              int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp,
+                                              unsigned total, float& f2max, float& viscmax, unsigned int& nbsum) {
   const int lane = threadIdx.x & 31, q = lane >> 3, r = lane & 7;
   const unsigned t0 = grp * 8 + 2 * q, t1 = t0 + 1;
   const bool act0 = t0 < n_a, act1 = t1 < n_a;
@@ -148,15 +187,17 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   // ---- state of the two a of this lane (inactive: far away, never accepted) ----
   PairA a;
   __half2 nx0, ny0, nz0, th0, nx1, ny1, nz1, th1;
+  float rho_a0, rho_a1;
   {
     float4 p0 = S.rpos[ja0], v0 = S.rvel[ja0], p1 = S.rpos[ja1], v1 = S.rvel[ja1];
     if (!act0) { p0 = make_float4(-Q_FAR, -Q_FAR, -Q_FAR, 1.f); v0 = make_float4(0.f, 0.f, 0.f, 0.f); }
     if (!act1) { p1 = make_float4(-Q_FAR, -Q_FAR, -Q_FAR, 1.f); v1 = make_float4(0.f, 0.f, 0.f, 0.f); }
-    a.x = make_float2(p0.x, p1.x); a.y = make_float2(p0.y, p1.y); a.z = make_float2(p0.z, p1.z);
-    a.rho = make_float2(p0.w, p1.w);
-    a.inv_rho = make_float2(fast_rcp(p0.w), fast_rcp(p1.w));
-    a.vx = make_float2(v0.x, v1.x); a.vy = make_float2(v0.y, v1.y); a.vz = make_float2(v0.z, v1.z);
-    a.P = make_float2(v0.w, v1.w);
+    a.x = f2_pack_pinned(p0.x, p1.x); a.y = f2_pack_pinned(p0.y, p1.y); a.z = f2_pack_pinned(p0.z, p1.z);
+    a.rho = f2_pack_pinned(p0.w, p1.w);
+    rho_a0 = p0.w; rho_a1 = p1.w;
+    a.inv_rho = f2_pack_pinned(fast_rcp(p0.w), fast_rcp(p1.w));
+    a.vx = f2_pack_pinned(v0.x, v1.x); a.vy = f2_pack_pinned(v0.y, v1.y); a.vz = f2_pack_pinned(v0.z, v1.z);
+    a.P = f2_pack_pinned(v0.w, v1.w);
     // prefilter operands (half precision): s = |b|^2 - 2 a.b  <  thr = R2u + margin - |a|^2
     const float thr0 = act0 ? (C.R2u + Q_MARGIN) - fmaf(p0.z, p0.z, fmaf(p0.y, p0.y, p0.x * p0.x)) : -60000.f;
     const float thr1 = act1 ? (C.R2u + Q_MARGIN) - fmaf(p1.z, p1.z, fmaf(p1.y, p1.y, p1.x * p1.x)) : -60000.f;
@@ -166,22 +207,25 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     nz1 = __float2half2_rn(act1 ? -2.f * p1.z : 0.f); th1 = __half2half2(__float2half_ru(thr1));
   }
   PairAcc2 acc;
-  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = make_float2(0.f, 0.f);
+  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = f2_pack(0.f, 0.f);
   acc.visc0 = acc.visc1 = 0.f;
   acc.nb0 = acc.nb1 = 0u;
 
-  const float ddtb = C.ddt_over_boundary ? 1.f : 0.f;
-  const int nruns = A_FLUID ? 18 : 9;      // fluid a: 9 boundary-block rows then 9 fluid rows; boundary a: fluid rows
+  // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
+  // term only if ddt_over_boundary, A4), then the 9 fluid rows; boundary a sweeps the fluid rows only (Eq. 36).
+  const int nruns = A_FLUID ? 18 : 9;
   int ri = 0;
   int gw = -1, g_first = 0, g_last = -1;
   unsigned j0 = 0, j1 = 0;
-  bool run_ddt = true;
+  const unsigned dummy_addr = total * 16u;
 
-  while (true) {
+  while (ri < nruns) {
     // ================= T phase: fill up to QW words =================
+    const int ri_end = (A_FLUID && ri < 9) ? 9 : nruns;
+    const float ddtw = (A_FLUID && ri < 9 && !C.ddt_over_boundary) ? 0.f : 1.f;
     int nw = 0;
     unsigned cnt = 0;
-    while (nw < QW && ri < nruns) {
+    while (nw < QW && ri < ri_end) {
       if (gw < 0) {   // open run ri
         const int blk_b = A_FLUID ? (ri >= 9 ? 1 : 0) : 1;
         const int k = ri % 9, iz = 1 + cz + (k / 3 - 1), iy = 1 + cy + (k % 3 - 1);
@@ -191,7 +235,6 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
         g_first = (int)(j0 >> 4);
         g_last = (int)((j1 - 1) >> 4);
         gw = g_first;
-        run_ddt = blk_b == 1 || C.ddt_over_boundary != 0;
       }
       const int nstep = min(16, g_last - gw + 1);
       const uint4* tp = S.tst + gw * 8 + r;
@@ -221,50 +264,51 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
         if (c + 8u >= j1) kill |= 0x10000u << il;
       }
       u &= ~kill;
-      bmw[nw * 32 + lane] = u;
-      if (lane == 0) descw[nw] = ((unsigned)gw * 16u) | (run_ddt ? 0x80000000u : 0u);
+      // word + byte address of the record of bit 0 (bit p -> + 256 (p & 15) + 128 (p >> 4))
+      bmw[nw * 32 + lane] = make_uint2(u, ((unsigned)gw * 16u + (unsigned)r) * 16u);
       cnt += (u != 0u) ? (unsigned)__popc(u) : 1u;   // a zero word costs one idle iteration
       nw++;
       gw += 16;
       if (gw > g_last) { ri++; gw = -1; }
     }
-    if (nw == 0) break;
+    if (nw == 0) continue;
     __syncwarp();
 
     // ================= P phase: every lane pops its own words =================
     const unsigned n_it = __reduce_max_sync(0xffffffffu, cnt);
-    unsigned cur = 0, base_r = 0;
+    unsigned cur = 0, base = 0;
     int wi = 0;
-    float ddtw = 0.f;
+    const unsigned char* rp = reinterpret_cast<const unsigned char*>(S.rpos);
+    const unsigned char* rv = reinterpret_cast<const unsigned char*>(S.rvel);
 #pragma unroll 2
     for (unsigned it = 0; it < n_it; it++) {
-      if (cur == 0u && wi < nw) {
-        cur = bmw[wi * 32 + lane];
-        const unsigned d = descw[wi];
-        base_r = (d & 0x7fffffffu) + (unsigned)r;
-        ddtw = (d >> 31) ? 1.f : ddtb;
-        wi++;
-      }
-      const int p = __ffs(cur) - 1;
-      const unsigned idx = cur != 0u ? base_r + (((unsigned)p & 15u) << 4) + (((unsigned)p >> 4) << 3) : total;
-      cur &= cur - 1u;
-      const float4 pb = S.rpos[idx];
-      const float4 vb = S.rvel[idx];
+      // reload (branch free): the word slot read is clamped, the result is used only if needed
+      const bool need = cur == 0u && wi < nw;
+      const uint2 e = bmw[min(wi, QW - 1) * 32 + lane];
+      cur = need ? e.x : cur;
+      base = need ? e.y : base;
+      wi += need ? 1 : 0;
+      // pop the highest set bit
+      const unsigned p = 31u - (unsigned)__clz((int)cur);          // cur == 0 -> p = 0xffffffff (unused)
+      const unsigned addr = cur != 0u ? base + ((p & 15u) << 8) + ((p >> 4) << 7) : dummy_addr;
+      cur &= ~(1u << (p & 31u));
+      const float4 pb = *reinterpret_cast<const float4*>(rp + addr);
+      const float4 vb = *reinterpret_cast<const float4*>(rv + addr);
       pair2<A_FLUID>(C, a, pb, vb, ddtw, acc);
     }
     __syncwarp();
-    if (ri >= nruns) break;
   }
 
   // ---- combine the 8 lanes of each quarter-warp; lane r = 0 writes both particles ----
-  acc.sc.x = qsum(acc.sc.x); acc.sc.y = qsum(acc.sc.y);
+  PairAcc r0 = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, r1 = r0;
+  r0.sc = qsum(f2_lo(acc.sc)); r1.sc = qsum(f2_hi(acc.sc));
   acc.nb0 = qsumu(acc.nb0); acc.nb1 = qsumu(acc.nb1);
   if (A_FLUID) {
-    acc.sx.x = qsum(acc.sx.x); acc.sx.y = qsum(acc.sx.y);
-    acc.sy.x = qsum(acc.sy.x); acc.sy.y = qsum(acc.sy.y);
-    acc.sz.x = qsum(acc.sz.x); acc.sz.y = qsum(acc.sz.y);
-    acc.sd.x = qsum(acc.sd.x); acc.sd.y = qsum(acc.sd.y);
-    acc.visc0 = qmax(acc.visc0); acc.visc1 = qmax(acc.visc1);
+    r0.sx = qsum(f2_lo(acc.sx)); r1.sx = qsum(f2_hi(acc.sx));
+    r0.sy = qsum(f2_lo(acc.sy)); r1.sy = qsum(f2_hi(acc.sy));
+    r0.sz = qsum(f2_lo(acc.sz)); r1.sz = qsum(f2_hi(acc.sz));
+    r0.sd = qsum(f2_lo(acc.sd)); r1.sd = qsum(f2_hi(acc.sd));
+    r0.visc = qmax(acc.visc0); r1.visc = qmax(acc.visc1);
   }
   if (r == 0) {
     const int ra = qrange(A_FLUID ? 1 : 0, 1 + cx, 1 + cy, 1 + cz);
@@ -272,14 +316,11 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
 #pragma unroll
     for (int h = 0; h < 2; h++) {
       if (h == 0 ? act0 : act1) {
-        PairAcc pa1;
-        pa1.sx = h ? acc.sx.y : acc.sx.x; pa1.sy = h ? acc.sy.y : acc.sy.x; pa1.sz = h ? acc.sz.y : acc.sz.x;
-        pa1.sc = h ? acc.sc.y : acc.sc.x; pa1.sd = h ? acc.sd.y : acc.sd.x;
-        pa1.visc = h ? acc.visc1 : acc.visc0;
+        const PairAcc& pa1 = h ? r1 : r0;
         unsigned nb = h ? acc.nb1 : acc.nb0;
         if (A_FLUID) nb -= 1u;   // the particle itself passed the test at r = 0 and contributed exactly 0 (A17)
         const unsigned ga = gbase + (h ? ja1 : ja0);
-        const float4 out = finish_particle(C, A_FLUID, h ? a.rho.y : a.rho.x, pa1);
+        const float4 out = finish_particle(C, A_FLUID, h ? rho_a1 : rho_a0, pa1);
         A.acc[ga] = out;
         if (A.nbcount) A.nbcount[ga] = nb;
         if (A_FLUID) f2max = fmaxf(f2max, fmaf(out.x, out.x, fmaf(out.y, out.y, out.z * out.z)));
@@ -298,9 +339,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   S.rpos = reinterpret_cast<float4*>(smem_raw);
   S.rvel = S.rpos + NMAX;
   S.tst = reinterpret_cast<uint4*>(S.rvel + NMAX);
-  S.bm = reinterpret_cast<uint32_t*>(S.tst + (NMAX / 16) * 8);
-  S.desc = S.bm + NWARP * QW * 32;
-  S.soff = S.desc + NWARP * QW;
+  S.bm = reinterpret_cast<uint2*>(S.tst + (NMAX / 16) * 8);
+  S.soff = reinterpret_cast<uint32_t*>(S.bm + NWARP * QW * 32);
   S.gstart = S.soff + (QNR + 1);
   S.seg = S.gstart + QNR;
   __shared__ uint32_t s_cnt[QNR];
@@ -435,8 +475,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   __syncthreads();
 
   // 4. a-groups, taken dynamically by the warps
-  uint32_t* bmw = S.bm + warp * QW * 32;
-  uint32_t* descw = S.desc + warp * QW;
+  uint2* bmw = S.bm + warp * QW * 32;
   while (true) {
     uint32_t gi = 0;
     if (lane == 0) gi = atomicAdd(&S.seg[0], 1u);
@@ -447,8 +486,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
     const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
     const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
-    if (blk == 1) process_group<true>(C, A, S, bmw, descw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
-    else process_group<false>(C, A, S, bmw, descw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    if (blk == 1) process_group<true>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    else process_group<false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
   }
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
@@ -458,7 +497,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
   constexpr int NWARP = NT / 32;
   const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint4) * (NMAX / 16) * 8 +
-                      sizeof(uint32_t) * (NWARP * QW * 32 + NWARP * QW + (QNR + 1) + QNR + (QNSEG + 2));
+                      sizeof(uint2) * NWARP * QW * 32 + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
