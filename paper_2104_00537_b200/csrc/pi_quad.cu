@@ -12,7 +12,7 @@
 //             one HSET2 per a evaluate the expanded-form prefilter |b|^2 - 2 a.b < R^2 + margin - |a|^2 for
 //             both candidates at once.  The prefilter is conservative (margin > its rounding error);
 //             the bits of both a are OR-ed into one 32-bit word per 16 steps and stored per lane.
-//   P phase : (pair) each lane pops its own words.  Every popped b is loaded once (two LDS.128, conflict free
+//   P phase : (pair) the lanes of a quarter-warp claim the stored words dynamically, in (word, residue) order.  Every popped b is loaded once (two LDS.128, conflict free
 //             because the 8 lanes of a quarter-warp hold 8 different residues) and evaluated against BOTH a of
 //             the lane with packed FP32x2 arithmetic, b entering as a broadcast scalar operand.  The exact
 //             canonical predicate C2 (fp32, individually rounded) decides membership; a b that is a neighbour
@@ -33,7 +33,7 @@ constexpr int QS = QT + 2;                // staged cells per axis
 constexpr int QNCELL = QS * QS * QS;      // 64 staged cells per type block
 constexpr int QNR = 2 * QNCELL;           // staged ranges: block 0 = boundary, block 1 = fluid
 constexpr int QNSEG = 2 * QT * QT * QT;   // a-segments: (block, centre cell)
-constexpr int QW = 9;                     // bitmap words per lane per round
+constexpr int QCAP = 64;                  // pool entries (non-empty words) per quarter-warp per round
 constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
 constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
 
@@ -45,7 +45,7 @@ struct QSmem {
   float4* rpos;       // (x, y, z, rho): exact tile-centred coordinates + density
   float4* rvel;       // (vx, vy, vz, P)
   uint4* tst;         // half2-packed test records: entry g*8 + r = candidates 16g+r (low halves) and 16g+r+8
-  uint2* bm;          // [warp][QW][32] (bitmap word, byte address of the record of its bit 0)
+  uint2* bm;          // [warp][4][QCAP] pools: (bitmap word, byte address of the record of its bit 0)
   uint32_t* soff;     // QNR + 1
   uint32_t* gstart;   // QNR
   uint32_t* seg;      // [0] group counter, [1..QNSEG+1] a-group prefix
@@ -82,6 +82,11 @@ __device__ __forceinline__ float f2_hi(f2 v) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
   return hi;
 }
+__device__ __forceinline__ float f_lt(float a, float b) {   // 1.0f if a < b else 0.0f
+  float r;
+  asm("set.lt.f32.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+  return r;
+}
 __device__ __forceinline__ f2 f2_add(f2 a, f2 b) {
   f2 r;
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
@@ -105,7 +110,7 @@ struct PairA {
 struct PairAcc2 {
   f2 sx, sy, sz, sc, sd;
   float visc0, visc1;
-  unsigned nb0, nb1;
+  f2 nb;              // neighbour counts, kept as floats (exact integers)
 };
 
 // One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free.  A b outside the
@@ -121,8 +126,7 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
   r2 = f2_fma(duy, duy, r2);
   r2 = f2_fma(duz, duz, r2);
   const float r2a = f2_lo(r2), r2b = f2_hi(r2);
-  A.nb0 += r2a < C.R2u ? 1u : 0u;
-  A.nb1 += r2b < C.R2u ? 1u : 0u;
+  A.nb = f2_add(A.nb, f2_pack(f_lt(r2a, C.R2u), f_lt(r2b, C.R2u)));   // exact: counts stay far below 2^24
   f2 w = f2_fma(f2_pack(fast_sqrt(r2a), fast_sqrt(r2b)), f2_bc(-C.qscale), f2_bc(1.0f));   // 1 - q/2   (Eq. 11)
   w = f2_pack(fmaxf(f2_lo(w), 0.f), fmaxf(f2_hi(w), 0.f));
   const f2 w3 = f2_mul(f2_mul(w, w), w);      // grad_a W_ab = Cf w^3 cs du
@@ -174,7 +178,7 @@ __device__ __forceinline__ unsigned qsumu(unsigned v) {
 }
 
 // One a-group: up to 8 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
-// A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw is this warp's bitmap area ([QW][32] uint2).
+// A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw is this warp's pool area ([4][QCAP] uint2).
 template <bool A_FLUID>
 __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint2* bmw, int cx,
                                               int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp,
@@ -207,9 +211,8 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     nz1 = __float2half2_rn(act1 ? -2.f * p1.z : 0.f); th1 = __half2half2(__float2half_ru(thr1));
   }
   PairAcc2 acc;
-  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = f2_pack(0.f, 0.f);
+  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = acc.nb = f2_pack(0.f, 0.f);
   acc.visc0 = acc.visc1 = 0.f;
-  acc.nb0 = acc.nb1 = 0u;
 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
   // term only if ddt_over_boundary, A4), then the 9 fluid rows; boundary a sweeps the fluid rows only (Eq. 36).
@@ -218,14 +221,17 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   int gw = -1, g_first = 0, g_last = -1;
   unsigned j0 = 0, j1 = 0;
   const unsigned dummy_addr = total * 16u;
+  uint2* bmq = bmw + q * QCAP;                       // pool of this quarter-warp
+  const unsigned qsel = 0x4440u | (unsigned)q;           // byte_perm selector: byte q of a ballot
+  const unsigned lt_mask = (1u << r) - 1u;               // lanes of the quarter-warp below this one
 
   while (ri < nruns) {
-    // ================= T phase: fill up to QW words =================
+    // ================= T phase: fill the pools (until one of them may overflow) =================
     const int ri_end = (A_FLUID && ri < 9) ? 9 : nruns;
     const float ddtw = (A_FLUID && ri < 9 && !C.ddt_over_boundary) ? 0.f : 1.f;
     int nw = 0;
-    unsigned cnt = 0;
-    while (nw < QW && ri < ri_end) {
+    unsigned npool = 0;
+    while (ri < ri_end && !__any_sync(0xffffffffu, npool + 8 > QCAP)) {
       if (gw < 0) {   // open run ri
         const int blk_b = A_FLUID ? (ri >= 9 ? 1 : 0) : 1;
         const int k = ri % 9, iz = 1 + cz + (k / 3 - 1), iy = 1 + cy + (k % 3 - 1);
@@ -264,9 +270,14 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
         if (c + 8u >= j1) kill |= 0x10000u << il;
       }
       u &= ~kill;
-      // word + byte address of the record of bit 0 (bit p -> + 256 (p & 15) + 128 (p >> 4))
-      bmw[nw * 32 + lane] = make_uint2(u, ((unsigned)gw * 16u + (unsigned)r) * 16u);
-      cnt += (u != 0u) ? (unsigned)__popc(u) : 1u;   // a zero word costs one idle iteration
+      // non-empty words go to the pool of this quarter-warp, compacted in (word, residue) order, together
+      // with the byte address of the record of bit 0 (bit p -> + 256 (p & 15) + 128 (p >> 4))
+      {
+        const unsigned nzq = __byte_perm(__ballot_sync(0xffffffffu, u != 0u), 0u, qsel);
+        if (u != 0u)
+          bmq[npool + (unsigned)__popc(nzq & lt_mask)] = make_uint2(u, ((unsigned)gw * 16u + (unsigned)r) * 16u);
+        npool += (unsigned)__popc(nzq);
+      }
       nw++;
       gw += 16;
       if (gw > g_last) { ri++; gw = -1; }
@@ -274,35 +285,50 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     if (nw == 0) continue;
     __syncwarp();
 
-    // ================= P phase: every lane pops its own words =================
-    const unsigned n_it = __reduce_max_sync(0xffffffffu, cnt);
-    unsigned cur = 0, base = 0;
-    int wi = 0;
+    // ================= P phase: the 8 lanes of a quarter-warp claim words from their pool =================
+    // Words are claimed in pool order, so the 8 words in flight are (nearly always) 8 consecutive pool entries
+    // = 8 different residues: the record loads stay bank-conflict free while the work is balanced dynamically.
     const unsigned char* rp = reinterpret_cast<const unsigned char*>(S.rpos);
     const unsigned char* rv = reinterpret_cast<const unsigned char*>(S.rvel);
-#pragma unroll 2
-    for (unsigned it = 0; it < n_it; it++) {
-      // reload (branch free): the word slot read is clamped, the result is used only if needed
-      const bool need = cur == 0u && wi < nw;
-      const uint2 e = bmw[min(wi, QW - 1) * 32 + lane];
-      cur = need ? e.x : cur;
-      base = need ? e.y : base;
-      wi += need ? 1 : 0;
-      // pop the highest set bit
-      const unsigned p = 31u - (unsigned)__clz((int)cur);          // cur == 0 -> p = 0xffffffff (unused)
-      const unsigned addr = cur != 0u ? base + ((p & 15u) << 8) + ((p >> 4) << 7) : dummy_addr;
-      cur &= ~(1u << (p & 31u));
-      const float4 pb = *reinterpret_cast<const float4*>(rp + addr);
-      const float4 vb = *reinterpret_cast<const float4*>(rv + addr);
-      pair2<A_FLUID>(C, a, pb, vb, ddtw, acc);
+    unsigned cur = 0, base = 0, next = 8;
+    if ((unsigned)r < npool) {
+      const uint2 e = bmq[r];
+      cur = e.x;
+      base = e.y;
     }
+    // one step: claim (branch free; lanes whose word is used up take the next pool entries in lane order),
+    // pop the highest set bit, load the record, evaluate.  Written twice per loop trip so that the
+    // accumulators ping-pong between registers without moves.
+#define Q_STEP                                                                                         \
+  {                                                                                                    \
+    const bool need = cur == 0u;                                                                       \
+    const unsigned nq = __byte_perm(__ballot_sync(0xffffffffu, need), 0u, qsel);                       \
+    const unsigned ei = next + (unsigned)__popc(nq & lt_mask);                                         \
+    next += (unsigned)__popc(nq);                                                                      \
+    const bool take = need && ei < npool;                                                              \
+    const uint2 e = bmq[min(ei, (unsigned)(QCAP - 1))];                                              \
+    cur = take ? e.x : cur;                                                                            \
+    base = take ? e.y : base;                                                                          \
+    if (!__any_sync(0xffffffffu, cur != 0u || next < npool)) break;                                    \
+    const unsigned p = 31u - (unsigned)__clz((int)cur); /* cur == 0 -> p = 0xffffffff (unused) */      \
+    const unsigned addr = cur != 0u ? base + ((p & 15u) << 8) + ((p >> 4) << 7) : dummy_addr;          \
+    cur &= ~(1u << (p & 31u));                                                                         \
+    const float4 pb = *reinterpret_cast<const float4*>(rp + addr);                                     \
+    const float4 vb = *reinterpret_cast<const float4*>(rv + addr);                                     \
+    pair2<A_FLUID>(C, a, pb, vb, ddtw, acc);                                                           \
+  }
+    while (true) {
+      Q_STEP
+      Q_STEP
+    }
+#undef Q_STEP
     __syncwarp();
   }
 
   // ---- combine the 8 lanes of each quarter-warp; lane r = 0 writes both particles ----
   PairAcc r0 = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, r1 = r0;
   r0.sc = qsum(f2_lo(acc.sc)); r1.sc = qsum(f2_hi(acc.sc));
-  acc.nb0 = qsumu(acc.nb0); acc.nb1 = qsumu(acc.nb1);
+  const unsigned nb0 = (unsigned)qsum(f2_lo(acc.nb)), nb1 = (unsigned)qsum(f2_hi(acc.nb));
   if (A_FLUID) {
     r0.sx = qsum(f2_lo(acc.sx)); r1.sx = qsum(f2_hi(acc.sx));
     r0.sy = qsum(f2_lo(acc.sy)); r1.sy = qsum(f2_hi(acc.sy));
@@ -317,7 +343,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     for (int h = 0; h < 2; h++) {
       if (h == 0 ? act0 : act1) {
         const PairAcc& pa1 = h ? r1 : r0;
-        unsigned nb = h ? acc.nb1 : acc.nb0;
+        unsigned nb = h ? nb1 : nb0;
         if (A_FLUID) nb -= 1u;   // the particle itself passed the test at r = 0 and contributed exactly 0 (A17)
         const unsigned ga = gbase + (h ? ja1 : ja0);
         const float4 out = finish_particle(C, A_FLUID, h ? rho_a1 : rho_a0, pa1);
@@ -340,7 +366,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   S.rvel = S.rpos + NMAX;
   S.tst = reinterpret_cast<uint4*>(S.rvel + NMAX);
   S.bm = reinterpret_cast<uint2*>(S.tst + (NMAX / 16) * 8);
-  S.soff = reinterpret_cast<uint32_t*>(S.bm + NWARP * QW * 32);
+  S.soff = reinterpret_cast<uint32_t*>(S.bm + NWARP * 4 * QCAP);
   S.gstart = S.soff + (QNR + 1);
   S.seg = S.gstart + QNR;
   __shared__ uint32_t s_cnt[QNR];
@@ -402,7 +428,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   if (tid == 0) {
     uint32_t run = 0;
     for (int s = 0; s < QNSEG; s++) {
-      const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
+      const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
       uint32_t n = 0;
       if (cx < vx && cy < vy && cz < vz) n = s_cnt[qrange(blk, 1 + cx, 1 + cy, 1 + cz)];
       S.seg[1 + s] = run;
@@ -422,7 +448,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   if (total + 1 > (uint32_t)NMAX) {
     // staged set does not fit in shared memory (very crowded cells): per-particle global gather
     for (int s = 0; s < QNSEG; s++) {
-      const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
+      const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
       if (cx >= vx || cy >= vy || cz >= vz) continue;
       const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
       const uint32_t g0 = S.gstart[rr], len = s_cnt[rr];
@@ -475,7 +501,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   __syncthreads();
 
   // 4. a-groups, taken dynamically by the warps
-  uint2* bmw = S.bm + warp * QW * 32;
+  uint2* bmw = S.bm + warp * 4 * QCAP;
   while (true) {
     uint32_t gi = 0;
     if (lane == 0) gi = atomicAdd(&S.seg[0], 1u);
@@ -483,7 +509,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     if (gi >= ngroups) break;
     int s = 0;
     while (s + 1 < QNSEG && gi >= S.seg[1 + s + 1]) s++;
-    const int blk = s >> 3, cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
+    const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
     const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
     const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
     if (blk == 1) process_group<true>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
@@ -497,7 +523,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
   constexpr int NWARP = NT / 32;
   const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint4) * (NMAX / 16) * 8 +
-                      sizeof(uint2) * NWARP * QW * 32 + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
+                      sizeof(uint2) * NWARP * 4 * QCAP + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
@@ -521,5 +547,5 @@ int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.dim != 3 || C.k != 1) return -1;
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
-  return launch_quad<384, 4992>(C, A, s);
+  return launch_quad<512, 4928>(C, A, s);
 }
