@@ -34,6 +34,7 @@ constexpr int QNCELL = QS * QS * QS;      // 64 staged cells per type block
 constexpr int QNR = 2 * QNCELL;           // staged ranges: block 0 = boundary, block 1 = fluid
 constexpr int QNSEG = 2 * QT * QT * QT;   // a-segments: (block, centre cell)
 constexpr int QCAP = 64;                  // pool entries (non-empty words) per quarter-warp per round
+constexpr int QB = 4;                     // T-phase steps whose loads are issued together
 constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
 constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
 
@@ -245,17 +246,25 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       const int nstep = min(16, g_last - gw + 1);
       const uint4* tp = S.tst + gw * 8 + r;
       unsigned u = 0;
+      // 16 steps in batches of QB: the loads of a batch are issued together (clamped to the last valid step,
+      // the surplus bits are masked below), so that they overlap the arithmetic of the previous batch
 #pragma unroll
-      for (int i = 0; i < 16; i++) {
-        if (i < nstep) {
-          const uint4 t = tp[i * 8];
-          const __half2 bx = u32_as_h2(t.x), by = u32_as_h2(t.y), bz = u32_as_h2(t.z), bw = u32_as_h2(t.w);
-          const __half2 s0 = __hfma2(nz0, bz, __hfma2(ny0, by, __hfma2(nx0, bx, bw)));
-          const __half2 s1 = __hfma2(nz1, bz, __hfma2(ny1, by, __hfma2(nx1, bx, bw)));
-          const unsigned m = __hlt2_mask(s0, th0) | __hlt2_mask(s1, th1);
-          u |= m & (0x00010001u << i);
+      for (int b0 = 0; b0 < 16; b0 += QB) {
+        if (b0 < nstep) {
+          uint4 t[QB];
+#pragma unroll
+          for (int i = 0; i < QB; i++) t[i] = tp[min(b0 + i, nstep - 1) * 8];
+#pragma unroll
+          for (int i = 0; i < QB; i++) {
+            const __half2 bx = u32_as_h2(t[i].x), by = u32_as_h2(t[i].y), bz = u32_as_h2(t[i].z), bw = u32_as_h2(t[i].w);
+            const __half2 s0 = __hfma2(nz0, bz, __hfma2(ny0, by, __hfma2(nx0, bx, bw)));
+            const __half2 s1 = __hfma2(nz1, bz, __hfma2(ny1, by, __hfma2(nx1, bx, bw)));
+            const unsigned m = __hlt2_mask(s0, th0) | __hlt2_mask(s1, th1);
+            u |= m & (0x00010001u << (b0 + i));
+          }
         }
       }
+      u &= (0xffffu >> (16 - nstep)) * 0x00010001u;
       // candidates of the first / last group that lie outside the run [j0, j1)
       unsigned kill = 0;
       if (gw == g_first) {
