@@ -218,7 +218,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
   // term only if ddt_over_boundary, A4), then the 9 fluid rows; boundary a sweeps the fluid rows only (Eq. 36).
   const int nruns = A_FLUID ? 18 : 9;
-  int ri = 0;
+  int ri = (A_FLUID && S.soff[QNCELL] == 0u) ? 9 : 0;   // no boundary particle staged: skip their 9 rows
   int gw = -1, g_first = 0, g_last = -1;
   unsigned j0 = 0, j1 = 0;
   const unsigned dummy_addr = total * 16u;
@@ -383,6 +383,21 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int tx = blockIdx.x % ntx, ty = (blockIdx.x / ntx) % nty, tz = blockIdx.x / (ntx * nty);
   const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
+
+  // 0. most tiles of a dam break are air: leave early if the centre cells hold no particle.  x-adjacent
+  //    cells are adjacent keys, so one (block, cy, cz) row of centre cells is one cellstart difference.
+  {
+    bool any = false;
+    if (tid < 2 * QT * QT) {
+      const int blk = tid / (QT * QT), cz = oz + (tid / QT) % QT, cy = oy + tid % QT;
+      if (cy < C.nc[1] && cz < C.nc[2]) {
+        const uint32_t key = (uint32_t)blk * C.ncells + (uint32_t)ox +
+                             (uint32_t)C.nc[0] * ((uint32_t)cy + (uint32_t)C.nc[1] * (uint32_t)cz);
+        any = A.cellstart[key + (uint32_t)min(QT, C.nc[0] - ox)] != A.cellstart[key];
+      }
+    }
+    if (!__syncthreads_or(any)) return;
+  }
 
   // 1. global ranges of the staged cells (both type blocks)
   for (int rr = tid; rr < QNR; rr += NT) {
