@@ -44,7 +44,7 @@ __device__ __forceinline__ int qrange(int blk, int ix, int iy, int iz) {   // st
 
 struct QSmem {
   float4* rpos;       // (x, y, z, rho): exact tile-centred coordinates + density
-  float4* rvel;       // (vx, vy, vz, P)
+  float4* rvel;       // (vx, vy, vz, P / rho)
   uint4* tst;         // half2-packed test records: entry g*8 + r = candidates 16g+r (low halves) and 16g+r+8
   uint2* bm;          // [warp][4][QCAP] pools: (bitmap word, byte address of the record of its bit 0)
   uint32_t* soff;     // QNR + 1
@@ -106,7 +106,7 @@ __device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
 
 // Packed state of the two particles a of a lane.
 struct PairA {
-  f2 x, y, z, vx, vy, vz, rho, inv_rho, P;
+  f2 x, y, z, vx, vy, vz, rho, inv_rho, kap;   // kap = P / rho
 };
 struct PairAcc2 {
   f2 sx, sy, sz, sc, sd;
@@ -116,10 +116,11 @@ struct PairAcc2 {
 
 // One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free.  A b outside the
 // support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record) gets weight 0:
-// w = max(1 - q/2, 0).  nb counts the exact canonical predicate C2.
-template <bool A_FLUID>
+// w = max(1 - q/2, 0).  nb counts the exact canonical predicate C2.  pb = (x, y, z, rho_b), vb = (v_b, P_b/rho_b).
+// DDT: this b enters the density diffusion term (A4).
+template <bool A_FLUID, bool DDT>
 __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const float4 pb, const float4 vb,
-                                      float ddtw, PairAcc2& A) {
+                                      PairAcc2& A) {
   const f2 dux = f2_add(a.x, f2_bc(-pb.x));   // exact (C1)
   const f2 duy = f2_add(a.y, f2_bc(-pb.y));
   const f2 duz = f2_add(a.z, f2_bc(-pb.z));
@@ -141,21 +142,27 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
   const f2 gb = f2_mul(w3, f2_bc(inv_rho_b));
   A.sc = f2_fma(gb, dot, A.sc);
   if (A_FLUID) {
-    const f2 drho = f2_add(a.rho, f2_bc(-pb.w));
-    A.sd = f2_fma(f2_mul(gb, f2_bc(ddtw)), drho, A.sd);
+    if (DDT) A.sd = f2_fma(gb, f2_add(a.rho, f2_bc(-pb.w)), A.sd);
     const f2 rs = f2_add(a.rho, f2_bc(pb.w));
     const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), rs);
-    const f2 x = f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den)));
-    const f2 mu = f2_mul(dot, f2_mul(x, rs));             // mu_ab / c_mu   (Eq. 21, A12)
+    const f2 y = f2_mul(dot, f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den))));   // dot / ((r2 + eta2) rs)
+    const f2 mu = f2_mul(y, rs);                          // mu_ab / c_mu   (Eq. 21, A12)
     A.visc0 = fmaxf(A.visc0, fabsf(f2_lo(mu)));
     A.visc1 = fmaxf(A.visc1, fabsf(f2_hi(mu)));
-    const f2 t = f2_mul(f2_pack(fminf(f2_lo(dot), 0.f), fminf(f2_hi(dot), 0.f)), x);   // approaching pairs only
-    const f2 pp = f2_mul(f2_add(a.P, f2_bc(vb.w)), f2_mul(a.inv_rho, f2_bc(inv_rho_b)));
+    const f2 t = f2_pack(fminf(f2_lo(y), 0.f), fminf(f2_hi(y), 0.f));   // approaching pairs only (Eq. 21)
+    // (Pa + Pb) / (rho_a rho_b) = kap_a / rho_b + kap_b / rho_a
+    const f2 pp = f2_fma(a.kap, f2_bc(inv_rho_b), f2_mul(a.inv_rho, f2_bc(vb.w)));
     const f2 coef = f2_mul(w3, f2_fma(f2_bc(C.c_pi), t, pp));
     A.sx = f2_fma(coef, dux, A.sx);
     A.sy = f2_fma(coef, duy, A.sy);
     A.sz = f2_fma(coef, duz, A.sz);
   }
+}
+
+// Predicated 64-bit shared-memory load into an existing register pair (nothing happens if !p).
+__device__ __forceinline__ void lds64_if(bool p, unsigned saddr, unsigned& x, unsigned& y) {
+  asm volatile("{.reg .pred q; setp.ne.u32 q, %2, 0; @q ld.shared.v2.u32 {%0, %1}, [%3];}"
+               : "+r"(x), "+r"(y) : "r"((unsigned)p), "r"(saddr));
 }
 
 // Sum over the 8 lanes of a quarter-warp (butterfly, fixed order).
@@ -202,7 +209,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     rho_a0 = p0.w; rho_a1 = p1.w;
     a.inv_rho = f2_pack_pinned(fast_rcp(p0.w), fast_rcp(p1.w));
     a.vx = f2_pack_pinned(v0.x, v1.x); a.vy = f2_pack_pinned(v0.y, v1.y); a.vz = f2_pack_pinned(v0.z, v1.z);
-    a.P = f2_pack_pinned(v0.w, v1.w);
+    a.kap = f2_pack_pinned(v0.w, v1.w);
     // prefilter operands (half precision): s = |b|^2 - 2 a.b  <  thr = R2u + margin - |a|^2
     const float thr0 = act0 ? (C.R2u + Q_MARGIN) - fmaf(p0.z, p0.z, fmaf(p0.y, p0.y, p0.x * p0.x)) : -60000.f;
     const float thr1 = act1 ? (C.R2u + Q_MARGIN) - fmaf(p1.z, p1.z, fmaf(p1.y, p1.y, p1.x * p1.x)) : -60000.f;
@@ -223,13 +230,14 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   unsigned j0 = 0, j1 = 0;
   const unsigned dummy_addr = total * 16u;
   uint2* bmq = bmw + q * QCAP;                       // pool of this quarter-warp
+  const unsigned bmq_s = (unsigned)__cvta_generic_to_shared(bmq);
   const unsigned qsel = 0x4440u | (unsigned)q;           // byte_perm selector: byte q of a ballot
   const unsigned lt_mask = (1u << r) - 1u;               // lanes of the quarter-warp below this one
 
   while (ri < nruns) {
     // ================= T phase: fill the pools (until one of them may overflow) =================
     const int ri_end = (A_FLUID && ri < 9) ? 9 : nruns;
-    const float ddtw = (A_FLUID && ri < 9 && !C.ddt_over_boundary) ? 0.f : 1.f;
+    const bool ddt_round = !(A_FLUID && ri < 9 && !C.ddt_over_boundary);
     int nw = 0;
     unsigned npool = 0;
     while (ri < ri_end && !__any_sync(0xffffffffu, npool + 8 > QCAP)) {
@@ -305,32 +313,40 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       cur = e.x;
       base = e.y;
     }
-    // one step: claim (branch free; lanes whose word is used up take the next pool entries in lane order),
-    // pop the highest set bit, load the record, evaluate.  Written twice per loop trip so that the
-    // accumulators ping-pong between registers without moves.
-#define Q_STEP                                                                                         \
+    // one step: claim (lanes whose word is used up take the next pool entries in lane order), pop the highest
+    // set bit and issue the loads of its record; then evaluate the record fetched by the previous step
+    // (software pipeline, two steps per loop trip so that records and accumulators ping-pong without moves).
+    // Pool words are non-empty, so "no word" means "pool used up"; a lane without work loads the dummy record.
+#define Q_FETCH(PB, VB)                                                                                \
   {                                                                                                    \
     const bool need = cur == 0u;                                                                       \
     const unsigned nq = __byte_perm(__ballot_sync(0xffffffffu, need), 0u, qsel);                       \
     const unsigned ei = next + (unsigned)__popc(nq & lt_mask);                                         \
     next += (unsigned)__popc(nq);                                                                      \
-    const bool take = need && ei < npool;                                                              \
-    const uint2 e = bmq[min(ei, (unsigned)(QCAP - 1))];                                              \
-    cur = take ? e.x : cur;                                                                            \
-    base = take ? e.y : base;                                                                          \
-    if (!__any_sync(0xffffffffu, cur != 0u || next < npool)) break;                                    \
+    lds64_if(need && ei < npool, bmq_s + ei * 8u, cur, base);                                          \
+    more = __any_sync(0xffffffffu, cur != 0u);                                                         \
     const unsigned p = 31u - (unsigned)__clz((int)cur); /* cur == 0 -> p = 0xffffffff (unused) */      \
     const unsigned addr = cur != 0u ? base + ((p & 15u) << 8) + ((p >> 4) << 7) : dummy_addr;          \
     cur &= ~(1u << (p & 31u));                                                                         \
-    const float4 pb = *reinterpret_cast<const float4*>(rp + addr);                                     \
-    const float4 vb = *reinterpret_cast<const float4*>(rv + addr);                                     \
-    pair2<A_FLUID>(C, a, pb, vb, ddtw, acc);                                                           \
+    PB = *reinterpret_cast<const float4*>(rp + addr);                                                  \
+    VB = *reinterpret_cast<const float4*>(rv + addr);                                                  \
   }
-    while (true) {
-      Q_STEP
-      Q_STEP
-    }
-#undef Q_STEP
+#define Q_LOOP(DDT)                                                                                    \
+  {                                                                                                    \
+    float4 pbA, vbA, pbB, vbB;                                                                         \
+    bool more;                                                                                         \
+    Q_FETCH(pbA, vbA)                                                                                  \
+    while (more) {                                                                                     \
+      Q_FETCH(pbB, vbB)                                                                                \
+      pair2<A_FLUID, DDT>(C, a, pbA, vbA, acc);                                                        \
+      if (!more) break;                                                                                \
+      Q_FETCH(pbA, vbA)                                                                                \
+      pair2<A_FLUID, DDT>(C, a, pbB, vbB, acc);                                                        \
+    }                                                                                                  \
+  }
+    if (ddt_round) Q_LOOP(true) else Q_LOOP(false)
+#undef Q_LOOP
+#undef Q_FETCH
     __syncwarp();
   }
 
@@ -495,7 +511,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
       const float4 p = A.posu[g0 + i];
       const float4 v = A.velp[g0 + i];
       S.rpos[d0 + i] = make_float4(p.x + fx, p.y + fy, p.z + fz, p.w);
-      S.rvel[d0 + i] = v;
+      S.rvel[d0 + i] = make_float4(v.x, v.y, v.z, __fdiv_rn(v.w, p.w));   // (v, P / rho)
     }
   }
   if (tid == 0) {   // dummy record: popped by lanes that have run out of work, never within any support
