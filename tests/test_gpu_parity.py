@@ -143,6 +143,55 @@ def test_config2_dambreak3d_scaled(sph, pi_kernel):
     check_one_pass(sph, developed_state(c, 3), pi_kernel)
 
 
+def test_config2_full_size_bench_configuration(sph):
+    """BASELINE.json configs[2] at full size (4.07 M fluid + 0.80 M boundary), in the launch configuration that
+    bench.py times (pi_kernel auto -> quad kernel): every particle against the oracle, on a state with seeded
+    velocity and density perturbations (v ~ N(0, 0.02 c0), rho = rho0 (1 + N(0, 1e-3)), the config-3 recipe)
+    so that all terms of Eq. 15-22 are exercised."""
+    c = wl.config(2)
+    n = len(c.rho)
+    idx = np.arange(n)
+    fluid = c.ptype == 0
+    vel = np.stack([wl.normal01(77, idx, k) for k in range(3)], 1) * (0.02 * c.params["c0"])
+    vel[~fluid] = 0.0
+    rho = c.params["rho0"] * (1.0 + 1e-3 * wl.normal01(77, idx, 3))
+    case = wl.Case(c.name + "_perturbed", c.pos, vel.astype(np.float32), rho.astype(np.float32), c.ptype, c.params)
+    info = check_one_pass(sph, case, 0)
+    assert info.pi_kernel == 3
+    assert info.n_interactions > 1_200_000_000
+
+
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_borderline_shells(sph, pi_kernel):
+    """Neighbour counts stay bit exact when many pairs sit within 1e-3 .. 1e-6 of the support radius, with the
+    particles a at the corners of the 2x2x2-cell tiles where the staged coordinates are largest (the quad
+    kernel's half-precision prefilter must never lose a true neighbour; C2 decides in fp32)."""
+    p = small_params()
+    cs = 2.0 * p["h"]
+    na, per = 48, 160
+    ia = np.arange(na)
+    # a: near cell corners, spread over the domain (cells 1..4 per axis, every second one a tile corner)
+    corner = np.stack([1 + (ia % 4), 1 + (ia // 4) % 4, 1 + (ia // 16) % 3], 1).astype(np.float64)
+    eps = 0.02 * (np.stack([wl.uniform01(21, ia, k) for k in range(3)], 1) - 0.5)
+    pa = (corner + eps) * cs
+    ib = np.arange(na * per)
+    z = 2.0 * wl.uniform01(22, ib, 0) - 1.0
+    ph = 2.0 * np.pi * wl.uniform01(22, ib, 1)
+    dirs = np.stack([np.sqrt(1 - z * z) * np.cos(ph), np.sqrt(1 - z * z) * np.sin(ph), z], 1)
+    rel = np.array([1 - 1e-3, 1 - 1e-4, 1 - 1e-5, 1 - 1e-6, 1 + 1e-6, 1 + 1e-5, 1 + 1e-4, 1 + 1e-3])[ib % 8]
+    pb = np.repeat(pa, per, axis=0) + dirs * (rel * cs)[:, None]
+    pos = np.concatenate([pa, pb])
+    inside = np.all((pos > 0.0) & (pos < 0.5), axis=1)
+    pos = pos[inside]
+    n = len(pos)
+    idx = np.arange(n)
+    vel = (0.2 * np.stack([wl.normal01(23, idx, k) for k in range(3)], 1)).astype(np.float32)
+    rho = (1000 * (1 + 0.005 * wl.normal01(23, idx, 3))).astype(np.float32)
+    typ = (wl.uniform01(23, idx, 4) < 0.2).astype(np.uint8)
+    info = check_one_pass(sph, wl.Case("shells", pos, vel, rho, typ, p), pi_kernel)
+    assert info.n_interactions > 2000
+
+
 # ---- edge cases ---------------------------------------------------------------------------------------
 def small_params(**kw):
     p = wl._params(3, 0.02, 1.2, 17.0, (0, 0, -9.81), (0, 0, 0), (0.5, 0.5, 0.5))
