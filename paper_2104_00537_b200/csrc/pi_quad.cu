@@ -103,6 +103,13 @@ __device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
   return r;
 }
+// acc += a * b, in place (input and output tied to one register pair: no moves around loop-carried sums)
+__device__ __forceinline__ void f2_fma_acc(f2 a, f2 b, f2& acc) {
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ void f2_add_acc(f2 a, f2& acc) {
+  asm("add.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(a));
+}
 
 // Packed state of the two particles a of a lane.
 struct PairA {
@@ -128,7 +135,7 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
   r2 = f2_fma(duy, duy, r2);
   r2 = f2_fma(duz, duz, r2);
   const float r2a = f2_lo(r2), r2b = f2_hi(r2);
-  A.nb = f2_add(A.nb, f2_pack(f_lt(r2a, C.R2u), f_lt(r2b, C.R2u)));   // exact: counts stay far below 2^24
+  f2_add_acc(f2_pack(f_lt(r2a, C.R2u), f_lt(r2b, C.R2u)), A.nb);   // exact: counts stay far below 2^24
   f2 w = f2_fma(f2_pack(fast_sqrt(r2a), fast_sqrt(r2b)), f2_bc(-C.qscale), f2_bc(1.0f));   // 1 - q/2   (Eq. 11)
   w = f2_pack(fmaxf(f2_lo(w), 0.f), fmaxf(f2_hi(w), 0.f));
   const f2 w3 = f2_mul(f2_mul(w, w), w);      // grad_a W_ab = Cf w^3 cs du
@@ -140,9 +147,9 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
   dot = f2_fma(dvy, duy, dot);
   dot = f2_fma(dvz, duz, dot);
   const f2 gb = f2_mul(w3, f2_bc(inv_rho_b));
-  A.sc = f2_fma(gb, dot, A.sc);
+  f2_fma_acc(gb, dot, A.sc);
   if (A_FLUID) {
-    if (DDT) A.sd = f2_fma(gb, f2_add(a.rho, f2_bc(-pb.w)), A.sd);
+    if (DDT) f2_fma_acc(gb, f2_add(a.rho, f2_bc(-pb.w)), A.sd);
     const f2 rs = f2_add(a.rho, f2_bc(pb.w));
     const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), rs);
     const f2 y = f2_mul(dot, f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den))));   // dot / ((r2 + eta2) rs)
@@ -153,9 +160,9 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
     // (Pa + Pb) / (rho_a rho_b) = kap_a / rho_b + kap_b / rho_a
     const f2 pp = f2_fma(a.kap, f2_bc(inv_rho_b), f2_mul(a.inv_rho, f2_bc(vb.w)));
     const f2 coef = f2_mul(w3, f2_fma(f2_bc(C.c_pi), t, pp));
-    A.sx = f2_fma(coef, dux, A.sx);
-    A.sy = f2_fma(coef, duy, A.sy);
-    A.sz = f2_fma(coef, duz, A.sz);
+    f2_fma_acc(coef, dux, A.sx);
+    f2_fma_acc(coef, duy, A.sy);
+    f2_fma_acc(coef, duz, A.sz);
   }
 }
 
@@ -336,10 +343,9 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     float4 pbA, vbA, pbB, vbB;                                                                         \
     bool more;                                                                                         \
     Q_FETCH(pbA, vbA)                                                                                  \
-    while (more) {                                                                                     \
+    while (more) { /* single exit: at most one surplus evaluation of dummy records per round */        \
       Q_FETCH(pbB, vbB)                                                                                \
       pair2<A_FLUID, DDT>(C, a, pbA, vbA, acc);                                                        \
-      if (!more) break;                                                                                \
       Q_FETCH(pbA, vbA)                                                                                \
       pair2<A_FLUID, DDT>(C, a, pbB, vbB, acc);                                                        \
     }                                                                                                  \
