@@ -38,6 +38,9 @@ constexpr int QB = 4;                     // T-phase steps whose loads are issue
 constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
 constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
 
+// offset of the staged range of row k = (dz + 1) * 3 + (dy + 1) relative to the row dy = dz = 0
+__constant__ int c_rowoff[9] = {-QS * QS - QS, -QS * QS, -QS * QS + QS, -QS, 0, QS, QS * QS - QS, QS * QS, QS * QS + QS};
+
 __device__ __forceinline__ int qrange(int blk, int ix, int iy, int iz) {   // staged indices, 0-based
   return ((blk * QS + iz) * QS + iy) * QS + ix;
 }
@@ -236,6 +239,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   int gw = -1, g_first = 0, g_last = -1;
   unsigned j0 = 0, j1 = 0;
   const unsigned dummy_addr = total * 16u;
+  const int row0 = qrange(1, cx, 1 + cy, 1 + cz);        // fluid-block range of the cell left of the centre cell
   uint2* bmq = bmw + q * QCAP;                       // pool of this quarter-warp
   const unsigned bmq_s = (unsigned)__cvta_generic_to_shared(bmq);
   const unsigned qsel = 0x4440u | (unsigned)q;           // byte_perm selector: byte q of a ballot
@@ -249,10 +253,10 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     unsigned npool = 0;
     while (ri < ri_end && !__any_sync(0xffffffffu, npool + 8 > QCAP)) {
       if (gw < 0) {   // open run ri
-        const int blk_b = A_FLUID ? (ri >= 9 ? 1 : 0) : 1;
-        const int k = ri % 9, iz = 1 + cz + (k / 3 - 1), iy = 1 + cy + (k % 3 - 1);
-        j0 = S.soff[qrange(blk_b, cx, iy, iz)];
-        j1 = S.soff[qrange(blk_b, cx + 2, iy, iz) + 1];
+        // row ri of the stencil: cells (cx-1 .. cx+1, cy+dy, cz+dz) of one type block are one contiguous range
+        const int row = ((A_FLUID && ri < 9) ? row0 - QNCELL : row0) + c_rowoff[(A_FLUID && ri >= 9) ? ri - 9 : ri];
+        j0 = S.soff[row];
+        j1 = S.soff[row + 3];
         if (j1 <= j0) { ri++; continue; }
         g_first = (int)(j0 >> 4);
         g_last = (int)((j1 - 1) >> 4);
@@ -261,14 +265,15 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       const int nstep = min(16, g_last - gw + 1);
       const uint4* tp = S.tst + gw * 8 + r;
       unsigned u = 0;
-      // 16 steps in batches of QB: the loads of a batch are issued together (clamped to the last valid step,
-      // the surplus bits are masked below), so that they overlap the arithmetic of the previous batch
+      // 16 steps in batches of QB: the loads of a batch are issued together, so that they overlap the
+      // arithmetic of the previous batch.  Steps beyond nstep read whatever follows (the test records are
+      // followed by the pools in shared memory, so the addresses stay valid); their bits are masked below.
 #pragma unroll
       for (int b0 = 0; b0 < 16; b0 += QB) {
         if (b0 < nstep) {
           uint4 t[QB];
 #pragma unroll
-          for (int i = 0; i < QB; i++) t[i] = tp[min(b0 + i, nstep - 1) * 8];
+          for (int i = 0; i < QB; i++) t[i] = tp[(b0 + i) * 8];   // may run past the run (never past the pools)
 #pragma unroll
           for (int i = 0; i < QB; i++) {
             const __half2 bx = u32_as_h2(t[i].x), by = u32_as_h2(t[i].y), bz = u32_as_h2(t[i].z), bw = u32_as_h2(t[i].w);
