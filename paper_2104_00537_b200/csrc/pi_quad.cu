@@ -393,6 +393,27 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   }
 }
 
+// Active-tile list: most tiles of a dam break are air.  A tile is active if its centre cells hold a particle;
+// x-adjacent cells are adjacent keys, so one (block, cy, cz) row of centre cells is one cellstart difference.
+// ws[0] = number of active tiles, ws[1] = next tile to take (both zeroed before the launch), ws[4..] = tile ids.
+__global__ void __launch_bounds__(256) k_quad_tiles(DevConsts C, const uint32_t* __restrict__ cellstart, int ntx, int nty,
+                                                    int ntiles, uint32_t* ws) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ntiles) return;
+  const int ox = (t % ntx) * QT, oy = ((t / ntx) % nty) * QT, oz = (t / (ntx * nty)) * QT;
+  const uint32_t w = (uint32_t)min(QT, C.nc[0] - ox);
+  bool any = false;
+  for (int blk = 0; blk < 2; blk++)
+    for (int cz = oz; cz < min(oz + QT, C.nc[2]); cz++)
+      for (int cy = oy; cy < min(oy + QT, C.nc[1]); cy++) {
+        const uint32_t key = (uint32_t)blk * C.ncells + (uint32_t)ox +
+                             (uint32_t)C.nc[0] * ((uint32_t)cy + (uint32_t)C.nc[1] * (uint32_t)cz);
+        any = any || cellstart[key + w] != cellstart[key];
+      }
+  if (any) ws[4 + atomicAdd(&ws[0], 1u)] = (uint32_t)t;
+}
+
+// Persistent kernel: one CTA per SM takes active tiles from the list until it is used up.
 template <int NT, int NMAX>
 __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int ntx, int nty) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -406,25 +427,21 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   S.gstart = S.soff + (QNR + 1);
   S.seg = S.gstart + QNR;
   __shared__ uint32_t s_cnt[QNR];
+  __shared__ uint32_t s_tile;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tx = blockIdx.x % ntx, ty = (blockIdx.x / ntx) % nty, tz = blockIdx.x / (ntx * nty);
-  const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
+  const uint32_t n_active = A.tile_ws[0];
+  float f2max = 0.f, viscmax = 0.f;
+  unsigned int nbsum = 0;
 
-  // 0. most tiles of a dam break are air: leave early if the centre cells hold no particle.  x-adjacent
-  //    cells are adjacent keys, so one (block, cy, cz) row of centre cells is one cellstart difference.
-  {
-    bool any = false;
-    if (tid < 2 * QT * QT) {
-      const int blk = tid / (QT * QT), cz = oz + (tid / QT) % QT, cy = oy + tid % QT;
-      if (cy < C.nc[1] && cz < C.nc[2]) {
-        const uint32_t key = (uint32_t)blk * C.ncells + (uint32_t)ox +
-                             (uint32_t)C.nc[0] * ((uint32_t)cy + (uint32_t)C.nc[1] * (uint32_t)cz);
-        any = A.cellstart[key + (uint32_t)min(QT, C.nc[0] - ox)] != A.cellstart[key];
-      }
-    }
-    if (!__syncthreads_or(any)) return;
-  }
+ for (;;) {
+  __syncthreads();                                  // every warp is done with the previous tile's shared memory
+  if (tid == 0) s_tile = atomicAdd(&A.tile_ws[1], 1u);
+  __syncthreads();
+  if (s_tile >= n_active) break;
+  const int tile = (int)A.tile_ws[4 + s_tile];
+  const int tx = tile % ntx, ty = (tile / ntx) % nty, tz = tile / (ntx * nty);
+  const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
 
   // 1. global ranges of the staged cells (both type blocks)
   for (int rr = tid; rr < QNR; rr += NT) {
@@ -490,11 +507,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   }
   __syncthreads();
   const uint32_t ngroups = S.seg[1 + QNSEG];
-  if (ngroups == 0) return;                       // nothing to compute in this tile (air)
+  if (ngroups == 0) continue;                     // nothing to compute in this tile
   const uint32_t total = S.soff[QNR];
-
-  float f2max = 0.f, viscmax = 0.f;
-  unsigned int nbsum = 0;
 
   if (total + 1 > (uint32_t)NMAX) {
     // staged set does not fit in shared memory (very crowded cells): per-particle global gather
@@ -505,8 +519,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
       const uint32_t g0 = S.gstart[rr], len = s_cnt[rr];
       for (uint32_t i = tid; i < len; i += NT) gather_one<3>(C, A, g0 + i, blk == 1, f2max, viscmax, nbsum);
     }
-    reduce_scalars(A.sc, f2max, viscmax, nbsum);
-    return;
+    continue;
   }
 
   // 2. stage particles with tile-centred coordinates: u + integer cell offset - QT/2.  Exact: every value is a
@@ -566,6 +579,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     if (blk == 1) process_group<true>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
     else process_group<false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
   }
+ }   // tiles
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
 
@@ -585,12 +599,29 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
     configured = true;
   }
   const long long ntiles = (long long)ntx * nty * ntz;
-  if (ntiles > 0x7fffffffLL) return -1;
-  k_pi_quad<NT, NMAX><<<(unsigned)ntiles, NT, smem, s>>>(C, A, ntx, nty);
+  if (ntiles > 0x7fffffffLL || A.tile_ws == nullptr) return -1;
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) {
+      cudaGetLastError();
+      n_sm = 0;
+      return -1;
+    }
+  }
+  if (cudaMemsetAsync(A.tile_ws, 0, 4 * sizeof(uint32_t), s) != cudaSuccess) return -1;
+  k_quad_tiles<<<(unsigned)((ntiles + 255) / 256), 256, 0, s>>>(C, A.cellstart, ntx, nty, (int)ntiles, A.tile_ws);
+  k_pi_quad<NT, NMAX><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
   return 0;
 }
 
 }  // namespace
+
+size_t pi_quad_workspace_words(const DevConsts& C) {
+  const size_t ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
+  return 4 + ntx * nty * ntz;
+}
 
 // Returns 0 if the quad kernel was launched, -1 if this configuration is not supported (caller falls back to
 // the tiled kernel): 3-D, cells of size 2h (27-cell stencil), eta^2 > 0.

@@ -35,7 +35,7 @@ struct sph_ctx {
   uint32_t* nbcount = nullptr;
   uint32_t *key[2] = {nullptr, nullptr}, *idx[2] = {nullptr, nullptr};
   int sorted_buf = 0;
-  uint32_t *block_hist = nullptr, *digit_total = nullptr, *cellstart = nullptr;
+  uint32_t *block_hist = nullptr, *digit_total = nullptr, *cellstart = nullptr, *tile_ws = nullptr;
   uint32_t nkeys = 0;
   int key_bits = 0;
   DevScalars* sc = nullptr;
@@ -276,6 +276,7 @@ int run_pi(sph_ctx* ctx) {
   A.nbcount = ctx->prm.count_neighbours ? ctx->nbcount : nullptr;
   A.sc = ctx->sc;
   A.n = ctx->n;
+  A.tile_ws = ctx->tile_ws;
   bool done = false;
   if (ctx->pi_kernel == 3) {
     done = pi_quad(ctx->C, A, s) == 0;
@@ -286,7 +287,7 @@ int run_pi(sph_ctx* ctx) {
     pi_gather(ctx->C, A, s);
     if (ctx->pi_kernel == 2) ctx->pi_kernel = 1;   // configuration not supported by the tiled kernel
   }
-  ctx->n_launch += 2;
+  ctx->n_launch += ctx->pi_kernel == 3 ? 3 : 2;   // reset + PI kernel (+ the quad kernel's active-tile list)
   ctx->n_pi += 1;
   CK(cudaGetLastError());
   return SPH_OK;
@@ -331,7 +332,8 @@ SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
   ctx->cellstart = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * ((size_t)ctx->nkeys + 1));
   ctx->sc = (DevScalars*)dalloc(ctx, sizeof(DevScalars));
   ctx->digit_total = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * 256 * 4);
-  if (!ctx->cellstart || !ctx->sc || !ctx->digit_total) {
+  ctx->tile_ws = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * pi_quad_workspace_words(ctx->C));
+  if (!ctx->cellstart || !ctx->sc || !ctx->digit_total || !ctx->tile_ws) {
     free_all(ctx);
     delete ctx;
     return SPH_E_NOMEM;
@@ -362,7 +364,7 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
   cudaStream_t s = ctx->stream;
   if (n > ctx->cap || !ctx->acc) {            // (re)allocate particle storage
     cudaStreamSynchronize(s);
-    void* keep[] = {ctx->cellstart, ctx->sc, ctx->digit_total, ctx->d_motions};
+    void* keep[] = {ctx->cellstart, ctx->sc, ctx->digit_total, ctx->tile_ws, ctx->d_motions};
     std::vector<void*> old = ctx->allocs;
     for (void* p : old) {
       bool k = false;

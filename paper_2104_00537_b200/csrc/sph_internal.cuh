@@ -83,7 +83,9 @@ struct PiArgs {
   uint32_t* nbcount;           // may be NULL
   DevScalars* sc;
   int64_t n;
+  uint32_t* tile_ws;           // quad kernel work space: [0] number of active tiles, [1] next tile, [4..] tile list
 };
+size_t pi_quad_workspace_words(const DevConsts& C);   // size of tile_ws in 32-bit words
 void pi_gather(const DevConsts& C, const PiArgs& A, cudaStream_t s);
 int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s);   // returns 0, or -1 if unsupported config
 int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s);    // 3-D, cell_div 1 only; 0 or -1 likewise
