@@ -140,6 +140,21 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def aggregate_replicas(ms_local, units_local, dist=None, device="cpu"):
+    """Replicas-only multi-GPU accounting: every rank runs the same workload on its own
+    GPU with no data-path collective; the job's time is the MAX over ranks and its work the SUM over ranks.
+    Returns (ms_max, units_total / seconds).  Works with any torch.distributed backend (nccl on GPUs, gloo in
+    the CPU tests)."""
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    ms_max = float(t.item())
+    return ms_max, float(u.item()) / (ms_max * 1e-3)
+
+
 def run_ours(args):
     import torch
     from paper_2104_00537_b200 import sph
@@ -193,11 +208,7 @@ def run_ours(args):
     inter = int(i1.n_interactions_total) - int(i0.n_interactions_total)
     launches = int(tm1.n_kernel_launches) - int(tm0.n_kernel_launches)
     n_pi = int(tm1.n_interaction_passes) - int(tm0.n_interaction_passes)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * inter / (ms_max * 1e-3)
+    ms_max, value = aggregate_replicas(ms_total, inter, dist, "cuda")
 
     # ---- end to end through the C ABI with host buffers (pinned): H2D + step + D2H every step ----
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -225,10 +236,7 @@ def run_ours(args):
         e2e_step()
     ev1.record(stream)
     barrier()
-    t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * per_step_inter * e2e_steps / (float(t.item()) * 1e-3)
+    _, e2e_value = aggregate_replicas(ev0.elapsed_time(ev1), per_step_inter * e2e_steps, dist, "cuda")
 
     if rank != 0:
         S.close()
