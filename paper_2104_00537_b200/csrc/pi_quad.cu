@@ -284,21 +284,16 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
           }
         }
       }
-      u &= (0xffffu >> (16 - nstep)) * 0x00010001u;
-      // candidates of the first / last group that lie outside the run [j0, j1)
-      unsigned kill = 0;
-      if (gw == g_first) {
-        const unsigned c = (unsigned)gw * 16u + (unsigned)r;
-        if (c < j0) kill |= 1u;
-        if (c + 8u < j0) kill |= 0x10000u;
+      // keep the candidates that lie inside the run [j0, j1): bit i (low half) is candidate c + 16 i, bit
+      // 16 + i is candidate c + 8 + 16 i with c = 16 gw + r.  Branch free; this also drops the steps >= nstep.
+      {
+        const int c = gw * 16 + r;
+        const int lo0 = max(((int)j0 - c + 15) >> 4, 0), lo1 = min(max(((int)j1 - c + 15) >> 4, 0), 16);
+        const int hi0 = max(((int)j0 - c + 7) >> 4, 0), hi1 = min(max(((int)j1 - c + 7) >> 4, 0), 16);
+        const unsigned mlo = (0xffffu >> (16 - lo1)) & (0xffffu << lo0);
+        const unsigned mhi = (0xffffu >> (16 - hi1)) & (0xffffu << hi0);
+        u &= (mlo & 0xffffu) | (mhi << 16);
       }
-      if (g_last - gw < 16) {
-        const unsigned c = (unsigned)g_last * 16u + (unsigned)r;
-        const int il = g_last - gw;
-        if (c >= j1) kill |= 1u << il;
-        if (c + 8u >= j1) kill |= 0x10000u << il;
-      }
-      u &= ~kill;
       // non-empty words go to the pool of this quarter-warp, compacted in (word, residue) order, together
       // with the byte address of the record of bit 0 (bit p -> + 256 (p & 15) + 128 (p >> 4))
       {
