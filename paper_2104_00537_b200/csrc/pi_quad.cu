@@ -1,19 +1,21 @@
 // Particle interaction (PI) task, "quad" kernel for sm_100a: 3-D, cells of size 2h (cell_div = 1).
 //
-// Same tile staging as pi_tiled.cu (a CTA owns 2x2x2 cells and stages them plus a one-cell halo in shared
-// memory with exact tile-centred coordinates, C1/C2), but the work of a warp is organised so that every
-// shared-memory access of the hot loops is bank-conflict free and the pair arithmetic runs on packed
-// FP32x2 instructions (FFMA2/FADD2/FMUL2, new on sm_100):
+// A persistent CTA (one per SM) takes 2x2x2-cell tiles from a device-built list of non-empty tiles and stages each
+// tile plus a one-cell halo in shared memory with exact tile-centred coordinates (C1/C2 hold bit for bit).  The
+// work of a warp is organised so that every shared-memory access of the hot loops is bank-conflict free and the
+// pair arithmetic runs on packed FP32x2 instructions (FFMA2/FADD2/FMUL2, new on sm_100):
 //
 //   a-group : 8 particles a of one cell = 4 quarter-warps x 2.  Quarter-warp q owns the pair (a_2q, a_2q+1);
 //             its 8 lanes r = 0..7 own the candidates b whose staged index is congruent to r modulo 8.
-//   T phase : (test) lane (q, r) walks the candidate runs 16 candidates per step: one LDS.128 brings the
+//   T phase : (test) lane (q, r) walks the candidate rows 16 candidates per step: one LDS.128 brings the
 //             half-precision test records of candidates 16g+r and 16g+r+8 (packed as half2), three HFMA2 and
 //             one HSET2 per a evaluate the expanded-form prefilter |b|^2 - 2 a.b < R^2 + margin - |a|^2 for
-//             both candidates at once.  The prefilter is conservative (margin > its rounding error);
-//             the bits of both a are OR-ed into one 32-bit word per 16 steps and stored per lane.
-//   P phase : (pair) the lanes of a quarter-warp claim the stored words dynamically, in (word, residue) order.  Every popped b is loaded once (two LDS.128, conflict free
-//             because the 8 lanes of a quarter-warp hold 8 different residues) and evaluated against BOTH a of
+//             both candidates at once.  The prefilter is conservative (margin > its rounding error, DESIGN.md
+//             5.2); the bits of both a are OR-ed into one 32-bit word per 16 steps; non-empty words go to a pool
+//             per quarter-warp in shared memory.
+//   P phase : (pair) the lanes of a quarter-warp claim the pool words dynamically, in (word, residue) order, so
+//             the 8 records loaded by a quarter-warp in one step lie in 8 different bank groups (two conflict-free
+//             LDS.128 per popped b) while the work stays balanced.  Every popped b is evaluated against BOTH a of
 //             the lane with packed FP32x2 arithmetic, b entering as a broadcast scalar operand.  The exact
 //             canonical predicate C2 (fp32, individually rounded) decides membership; a b that is a neighbour
 //             of only one of the two a contributes exactly 0 to the other (the kernel weight is clamped at 0).
