@@ -178,7 +178,8 @@ def run_ours(args):
     case = make_case(args.config, cell_div)
     n = case.n
     stream = torch.cuda.current_stream()
-    S = sph.Sph(case.params, pi_kernel=args.pi_kernel, count_neighbours=False, stream=stream)
+    S = sph.Sph(dict(case.params, integrator=1 if args.integrator == "verlet" else 0), pi_kernel=args.pi_kernel,
+                count_neighbours=False, stream=stream)
     S.load_case(case)
     S.compute_interactions()
     info0 = S.get_info()
@@ -289,7 +290,7 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": case.name, "n_particles": n, "n_fluid": case.n_fluid, "n_boundary": case.n_bound,
-                       "cell_div": cell_div, "pi_kernel": int(info0.pi_kernel), "multi_gpu": "replicas only",
+                       "cell_div": cell_div, "pi_kernel": int(info0.pi_kernel), "integrator": args.integrator, "multi_gpu": "replicas only",
                        "l2": "per-step working set (~190 B/particle x 4.9 M = 0.9 GB) is larger than the 126 MB L2",
                        "interactions_per_pass_t0": per_pass0},
             "steps_per_s": args.steps / (ms_max * 1e-3),
@@ -316,6 +317,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2 = headline)")
     ap.add_argument("--cell-div", type=int, default=1)
     ap.add_argument("--pi-kernel", type=int, default=0)
+    ap.add_argument("--integrator", choices=["symplectic", "verlet"], default="symplectic",
+                    help="symplectic (default, the metric's configuration) or verlet (Eq. 30-31, one pass per step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -66,6 +66,10 @@ typedef struct sph_params {
   int32_t pi_kernel;         /* interaction kernel: 0 auto, 1 gather (thread/particle), 2 tiled smem, */
                              /*   3 quad (3-D, cell_div 1: conflict-free smem + packed FP32x2)       */
   int32_t count_neighbours;  /* 1: keep per-particle neighbour counts (SPH_NBCOUNT); costs a store   */
+  int32_t integrator;        /* 0: symplectic predictor-corrector, Eq. 33-34 (two passes per step);  */
+                             /*   1: Verlet, Eq. 30-31 (one pass per step)         */
+  int32_t verlet_steps;      /* N_S of Eq. 31: step k is corrective when k mod N_S == 0 (the first   */
+                             /*   step included); 0 -> 40 ("N_S ~ 40 is recommended")  */
   sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
   sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */
   void* user;                /* passed back to dev_alloc / dev_free                                  */

@@ -213,6 +213,36 @@ class State:
         return self
 
 
+    def step_verlet(self, nsteps: int, verlet_steps: int = 40, mode: int = 1):
+        """Verlet scheme, Eq. 30-31 (one interaction pass per step); keeps the state n-1 and the step counter."""
+        n = self.cell.shape[0]
+        if not hasattr(self, "vel_m1"):
+            self.vel_m1 = np.zeros_like(self.vel)
+            self.rho_m1 = np.zeros_like(self.rho)
+            self.kstep = 0
+        sp = make_params(self.p)
+        nm = len(self.motions)
+        mot = (OrcMotion * max(nm, 1))()
+        for i, m in enumerate(self.motions):
+            mot[i].group, mot[i].axis = int(m["group"]), int(m["axis"])
+            mot[i].stroke, mot[i].period, mot[i].phase = m["stroke"], m["period"], m["phase"]
+        t = C.c_double(self.t)
+        k = C.c_int64(self.kstep)
+        hist = np.zeros(nsteps, np.float64)
+        rc = lib().orc_step_verlet(C.byref(sp), C.c_int64(n), _ptr(self.cell, C.c_int32),
+                                   _ptr(self.u, C.c_float), _ptr(self.out, C.c_uint8),
+                                   _ptr(self.vel, C.c_double), _ptr(self.rho, C.c_double),
+                                   _ptr(self.vel_m1, C.c_double), _ptr(self.rho_m1, C.c_double),
+                                   _ptr(self.ptype, C.c_uint8), C.c_int(nsteps), C.c_int(verlet_steps),
+                                   C.byref(k), mot, C.c_int(nm), _ptr(self.pos0, C.c_double), C.byref(t),
+                                   _ptr(hist, C.c_double), C.c_int(mode))
+        assert rc == 0
+        self.t = t.value
+        self.kstep = k.value
+        self.dt_hist.extend(hist.tolist())
+        return self
+
+
 def num_threads() -> int:
     return lib().orc_num_threads()
 

@@ -3,7 +3,7 @@
  *
  * Plain, slow, double-precision CPU oracle for the hot path of the weakly compressible SPH
  * method of arxiv 2104.00537 (DualSPHysics v5.0 paper, /root/reference/PAPER.md):
- * neighbour search + particle interaction + variable dt + symplectic step.
+ * neighbour search + particle interaction + variable dt + symplectic step (+ the Verlet scheme, Eq. 30-31).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
  * may call this.  It shares no code with the CUDA library (paper_2104_00537_b200/csrc):
@@ -19,7 +19,8 @@
  * and sign/magnitude against the analytic Laplacian; continuity against an independently
  * computed moment matrix; uniform lattice F = g; worked two-particle example
  * (tests/golden/two_particle.txt); dt closed form; integrator closed forms (free fall,
- * Pade density); hydrostatic column.  Everything else (absolute per-particle values on the
+ * Pade density; Verlet free fall and corrective-step rule); hydrostatic column.  The Verlet density leapfrog has no
+ * closed form to pin it: "parity unpinned" for that line beyond the free-fall and N_S = 1 (Euler) cases.  Everything else (absolute per-particle values on the
  * configs) is pinned only by these plus oracle-vs-GPU agreement: "parity otherwise unpinned".
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py).
@@ -492,6 +493,65 @@ ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, ui
     *t += dt;
   }
   free(pos_n); free(vel_n); free(rho_n); free(F); free(R); free(nb);
+  return 0;
+}
+
+/* nsteps Verlet steps, Eq. 30-31: ONE interaction pass per step.
+ *   regular step  (Eq. 30): v^{n+1} = v^{n-1} + 2 dt F^n ; rho^{n+1} = rho^{n-1} + 2 dt R^n
+ *   corrective step (Eq. 31): v^{n+1} = v^n + dt F^n     ; rho^{n+1} = rho^n + dt R^n
+ *   both                    : r^{n+1} = r^n + dt v^n + dt^2/2 F^n
+ * Readings (A21): the step counter k starts at 0 at load; step k is corrective when
+ * k mod N_S == 0 -- which includes the very first step, where no state n-1 exists -- N_S = verlet_steps
+ * ("N_S ~ 40 is recommended"); dt is the variable dt of Eq. 35 from this step's pass, used as
+ * printed (2 dt^n) although Eq. 30 assumes a constant step; boundary particles integrate rho with the same
+ * formulas (as A11) and take r, v from the motion law at t + dt.
+ * vel_m1 (n x 3), rho_m1 (n): state n-1, in/out (ignored on corrective steps); *kstep: counter, in/out. */
+ORC_API int orc_step_verlet(const orc_params* p, int64_t n, int32_t* cell, float* u, uint8_t* out,
+                            double* vel, double* rho, double* vel_m1, double* rho_m1, const uint8_t* type,
+                            int nsteps, int verlet_steps, int64_t* kstep, const orc_motion* motions, int nmotions,
+                            const double* pos0, double* t, double* dt_hist, int mode) {
+  int ncell[3]; double cs;
+  orc_grid(p, &cs, ncell, NULL);
+  double* pos_n = (double*)malloc(sizeof(double) * 3 * (size_t)n);
+  double* F = (double*)malloc(sizeof(double) * 3 * (size_t)n);
+  double* R = (double*)malloc(sizeof(double) * (size_t)n);
+  uint32_t* nb = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)n);
+  double x[3];
+  for (int s = 0; s < nsteps; s++) {
+    double visc;
+    orc_position(p, n, cell, u, pos_n);
+    orc_interactions(p, n, cell, u, out, vel, rho, type, mode, F, R, nb, &visc, NULL);   /* F^n, R^n */
+    double dt = orc_dt(p, n, F, type, out, visc);
+    if (dt_hist) dt_hist[s] = dt;
+    const int corrective = (*kstep % verlet_steps) == 0;
+    for (int64_t a = 0; a < n; a++) {
+      if (out[a]) continue;
+      const double rho_n = rho[a];
+      if (type[a] == 0) {
+        for (int k = 0; k < 3; k++) {
+          const double vn = vel[3 * a + k], f = F[3 * a + k];
+          x[k] = pos_n[3 * a + k] + dt * vn + 0.5 * dt * dt * f;
+          vel[3 * a + k] = corrective ? vn + dt * f : vel_m1[3 * a + k] + 2.0 * dt * f;
+          vel_m1[3 * a + k] = vn;
+        }
+        canon1(p, ncell, cs, x, cell + 3 * a, u + 3 * a, out + a);
+      } else if (type[a] >= 2) {          /* boundary with imposed motion: law at t + dt */
+        for (int k = 0; k < 3; k++) { x[k] = pos0[3 * a + k]; vel[3 * a + k] = 0.0; }
+        for (int j = 0; j < nmotions; j++)
+          if (motions[j].group == type[a]) {
+            double d, vv; motion_at(&motions[j], *t + dt, &d, &vv);
+            x[motions[j].axis] += d; vel[3 * a + motions[j].axis] = vv;
+          }
+        canon1(p, ncell, cs, x, cell + 3 * a, u + 3 * a, out + a);
+      }
+      rho[a] = corrective ? rho_n + dt * R[a] : rho_m1[a] + 2.0 * dt * R[a];
+      if (type[a] != 0 && p->rho_bound_floor && rho[a] < p->rho0) rho[a] = p->rho0;   /* A10 */
+      rho_m1[a] = rho_n;
+    }
+    *kstep += 1;
+    *t += dt;
+  }
+  free(pos_n); free(F); free(R); free(nb);
   return 0;
 }
 

@@ -44,6 +44,8 @@ struct sph_ctx {
   std::vector<Motion> motions;
   Motion* d_motions = nullptr;
   int pi_kernel = 1;
+  int integrator = 0, verlet_steps = 40;
+  int64_t kstep = 0;          // Verlet step counter since the last load (Eq. 31 every verlet_steps)
 
   bool profiling = false;
   std::vector<EventPair> events;
@@ -154,6 +156,8 @@ int validate(const sph_params* p, std::string& why) {
   if (p->alpha < 0 || p->delta < 0 || p->eta2_coef < 0) return bad("alpha, delta, eta2_coef must be >= 0");
   if (p->cell_div < 1 || p->cell_div > 3) return bad("cell_div must be 1, 2 or 3");
   if (p->pi_kernel < 0 || p->pi_kernel > 3) return bad("pi_kernel must be 0, 1, 2 or 3");
+  if (p->integrator < 0 || p->integrator > 1) return bad("integrator must be 0 (symplectic) or 1 (Verlet)");
+  if (p->verlet_steps < 0) return bad("verlet_steps must be >= 0");
   const double cs_min = 2.0 * p->h / p->cell_div;
   if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
   for (int k = 0; k < 3; k++) {
@@ -328,6 +332,8 @@ SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
   ctx->key_bits = 0;
   for (uint32_t v = 2u * ctx->C.ncells; v; v >>= 1) ctx->key_bits++;
   if (ctx->key_bits == 0) ctx->key_bits = 1;
+  ctx->integrator = params->integrator;
+  ctx->verlet_steps = params->verlet_steps > 0 ? params->verlet_steps : 40;
   ctx->pi_kernel = params->pi_kernel == 0 ? 3 : params->pi_kernel;   // auto: quad -> tiled -> gather, falling back per call
   ctx->cellstart = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * ((size_t)ctx->nkeys + 1));
   ctx->sc = (DevScalars*)dalloc(ctx, sizeof(DevScalars));
@@ -418,6 +424,7 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
   dfree(ctx, d_type);
   ctx->n = n;
   ctx->loaded = true;
+  ctx->kstep = 0;
   ctx->nl_valid = false;
   return SPH_OK;
 }
@@ -443,7 +450,7 @@ SPH_EXPORT int sph_set_motion(sph_ctx* ctx, int32_t group, int32_t axis, double 
 SPH_EXPORT int sph_compute_interactions(sph_ctx* ctx) {
   if (!ctx) return SPH_E_BADARG;
   if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_compute_interactions before sph_load_particles");
-  int rc = build_nl(ctx, false);
+  int rc = build_nl(ctx, ctx->integrator == 1);   // Verlet: the state n-1 travels with every reorder
   if (rc != SPH_OK) return rc;
   rc = run_pi(ctx);
   if (rc != SPH_OK) return rc;
@@ -461,7 +468,26 @@ SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
   if (nsteps < 0) return fail(ctx, SPH_E_BADARG, "nsteps < 0");
   cudaStream_t s = ctx->stream;
   const int nm = ctx->has_moving ? (int)ctx->motions.size() : 0;
-  for (int it = 0; it < nsteps; it++) {
+  for (int it = 0; it < nsteps && ctx->integrator == 1; it++) {   // Verlet, Eq. 30-31: one pass per step
+    int rc;
+    if ((rc = build_nl(ctx, true)) != SPH_OK) return rc;         // NL at state n; carries (v, rho)^{n-1}
+    if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^n, R^n
+    {
+      PhaseTimer t(ctx, PH_DT);
+      su_compute_dt(ctx->C, ctx->sc, s);                         // dt^n (Eq. 35)
+      ctx->n_launch += 1;
+    }
+    {
+      PhaseTimer t(ctx, PH_UPDATE);
+      su_verlet(ctx->C, ctx->set[ctx->cur], ctx->acc, ctx->n, ctx->sc, ctx->d_motions, nm, ctx->pos0,
+                ctx->kstep % ctx->verlet_steps == 0, s);
+      ctx->n_launch += 2;
+    }
+    ctx->kstep++;
+    ctx->nl_valid = false;
+    CK(cudaGetLastError());
+  }
+  for (int it = 0; it < nsteps && ctx->integrator == 0; it++) {
     int rc;
     if ((rc = build_nl(ctx, false)) != SPH_OK) return rc;        // NL at state n
     if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^n, R^n

@@ -100,6 +100,9 @@ void su_predictor(const DevConsts& C, const ParticleSet& P, const float4* acc, i
                   const Motion* motions, int nmotions, const double* pos0, cudaStream_t s);
 void su_corrector(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
                   const Motion* motions, int nmotions, const double* pos0, cudaStream_t s);
+// Verlet step, Eq. 30-31: corrective != 0 selects Eq. 31.  State n-1 lives in P.vel_n = (v^{n-1}, rho^{n-1}).
+void su_verlet(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
+               const Motion* motions, int nmotions, const double* pos0, int corrective, cudaStream_t s);
 // scatter sorted-order fields back to original order for sph_read_state
 void su_unsort_pos(const DevConsts& C, const ParticleSet& P, int64_t n, double* pos_out, int* cell_out,
                    float* off_out, cudaStream_t s);

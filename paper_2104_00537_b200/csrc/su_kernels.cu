@@ -160,6 +160,54 @@ __global__ void k_predictor(DevConsts C, ParticleSet P, const float4* __restrict
   P.cell[i] = lin;
 }
 
+// NEXT-1, Verlet scheme, Eq. 30-31, one interaction pass per step:
+//   regular:    v^{n+1} = v^{n-1} + 2 dt F^n;  rho^{n+1} = rho^{n-1} + 2 dt R^n     (Eq. 30)
+//   corrective: v^{n+1} = v^n + dt F^n;        rho^{n+1} = rho^n + dt R^n           (Eq. 31, every N_S steps)
+//   both:       r^{n+1} = r^n + dt v^n + dt^2/2 F^n
+// P.vel_n holds (v^{n-1}, rho^{n-1}) on entry and (v^n, rho^n) on exit.  Boundary: rho only, + imposed motion.
+__global__ void k_verlet(DevConsts C, ParticleSet P, const float4* __restrict__ acc, int64_t n, DevScalars* sc,
+                         const Motion* __restrict__ motions, int nmotions, const double* __restrict__ pos0,
+                         int corrective) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int lin = P.cell[i];
+  if (lin < 0) return;
+  const double dtd = sc->dt;
+  const float dt = (float)dtd;
+  const float4 p = P.posu[i];      // r^n (offsets), rho^n
+  float4 v = P.velp[i];            // v^n
+  const float4 m1 = P.vel_n[i];    // v^{n-1}, rho^{n-1}
+  const float4 a = acc[i];         // F^n, R^n
+  const uint8_t ty = P.type[i];
+  if (!(isfinite(a.x) && isfinite(a.y) && isfinite(a.z) && isfinite(a.w))) atomicOr(&sc->flags, 1u);
+  P.vel_n[i] = make_float4(v.x, v.y, v.z, p.w);
+  float u[3] = {p.x, p.y, p.z};
+  if (ty == 0) {
+    const float s = dt * C.inv_cs, hs = 0.5f * dt * s;
+    float du[3] = {fmaf(hs, a.x, s * v.x), fmaf(hs, a.y, s * v.y), fmaf(hs, a.z, s * v.z)};
+    lin = advance_cell(C, lin, u, du);
+    if (corrective) {
+      v.x = fmaf(dt, a.x, v.x);
+      v.y = fmaf(dt, a.y, v.y);
+      v.z = fmaf(dt, a.z, v.z);
+    } else {
+      v.x = fmaf(2.0f * dt, a.x, m1.x);
+      v.y = fmaf(2.0f * dt, a.y, m1.y);
+      v.z = fmaf(2.0f * dt, a.z, m1.z);
+    }
+  } else if (ty >= 2 && nmotions > 0) {
+    float vv[3];
+    lin = moved_boundary(C, motions, nmotions, ty, pos0, P.id[i], sc->t + dtd, u, vv);
+    v.x = vv[0]; v.y = vv[1]; v.z = vv[2];
+  }
+  float rho = corrective ? fmaf(dt, a.w, p.w) : fmaf(2.0f * dt, a.w, m1.w);
+  if (ty != 0 && C.rho_bound_floor) rho = fmaxf(rho, C.rho0);
+  if (lin < 0) atomicAdd(&sc->n_out, 1u);
+  P.posu[i] = make_float4(u[0], u[1], u[2], rho);
+  P.velp[i] = v;
+  P.cell[i] = lin;
+}
+
 // a9, corrector:  v^{n+1} = v^n + dt F^{n+1/2};  r^{n+1} = r^n + dt (v^{n+1} + v^n)/2;
 // eps = -(R^{n+1/2}/rho^{n+1/2}) dt;  rho^{n+1} = rho^n (2 - eps)/(2 + eps)       (Eq. 33-34)
 __global__ void k_corrector(DevConsts C, ParticleSet P, const float4* __restrict__ acc, int64_t n, DevScalars* sc,
@@ -268,6 +316,12 @@ void su_predictor(const DevConsts& C, const ParticleSet& P, const float4* acc, i
 void su_corrector(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
                   const Motion* motions, int nmotions, const double* pos0, cudaStream_t s) {
   if (n > 0) k_corrector<<<grid_for(n, 256), 256, 0, s>>>(C, P, acc, n, sc, motions, nmotions, pos0);
+  k_advance_time<<<1, 1, 0, s>>>(sc);
+}
+
+void su_verlet(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
+               const Motion* motions, int nmotions, const double* pos0, int corrective, cudaStream_t s) {
+  if (n > 0) k_verlet<<<grid_for(n, 256), 256, 0, s>>>(C, P, acc, n, sc, motions, nmotions, pos0, corrective);
   k_advance_time<<<1, 1, 0, s>>>(sc);
 }
 

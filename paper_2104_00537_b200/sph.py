@@ -43,6 +43,8 @@ class SphParams(C.Structure):
         ("cell_size", C.c_double),
         ("pi_kernel", C.c_int32),
         ("count_neighbours", C.c_int32),
+        ("integrator", C.c_int32),
+        ("verlet_steps", C.c_int32),
         ("dev_alloc", ALLOC_FN),
         ("dev_free", FREE_FN),
         ("user", C.c_void_p),
@@ -135,6 +137,8 @@ class Sph:
         sp.periodic[:] = [int(x) for x in params["periodic"]]
         sp.pi_kernel = int(params.get("pi_kernel", pi_kernel))
         sp.count_neighbours = int(bool(count_neighbours))
+        sp.integrator = int(params.get("integrator", 0))
+        sp.verlet_steps = int(params.get("verlet_steps", 0))
         self._stream = stream if stream is not None else torch.cuda.current_stream()
         sp.cuda_stream = self._stream.cuda_stream
 

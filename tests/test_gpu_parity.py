@@ -335,3 +335,44 @@ def test_nan_is_flagged(sph):
         with pytest.raises(sph.SphError) as e:
             S.get_info()
         assert e.value.code == sph.SPH_E_NAN
+
+
+# ---- NEXT-1: Verlet scheme, Eq. 30-31 ---------------------------------------------------
+@pytest.mark.parametrize("verlet_steps", [4, 40])
+def test_config0_verlet_steps(sph, verlet_steps):
+    """12 Verlet steps (one interaction pass each) against the oracle's Eq. 30-31; with verlet_steps = 4 the run
+    contains three corrective (Eq. 31) steps, with 40 only the first one."""
+    c = wl.config(0)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).step_verlet(12, verlet_steps)
+    p = dict(c.params, integrator=1, verlet_steps=verlet_steps)
+    with sph.Sph(p) as S:
+        S.load_case(c)
+        S.step(12)
+        info = S.get_info()
+        assert info.steps_done == 12 and info.n_out == 0 and st.out.sum() == 0
+        assert info.t == pytest.approx(st.t, rel=1e-5)
+        err = np.abs(S.read_state(sph.SPH_POS) - st.pos).max()
+        assert err <= 1e-3 * c.params["dp"], err
+        rho = S.read_state(sph.SPH_RHO).astype(np.float64)
+        assert abs(rho.sum() - st.rho.sum()) <= 1e-6 * st.rho.sum()
+        assert_close("rho", rho, st.rho, rtol=1e-5, floor=0)
+        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-3, floor=1e-3)
+        tm = S.get_timings()
+        assert tm.n_nl_builds == 12 and tm.n_interaction_passes == 12      # one pass per step
+
+
+def test_verlet_moving_boundary_and_reload(sph):
+    """Verlet with an imposed boundary motion (Eq. 37), interleaved sph_compute_interactions calls (the state n-1
+    must survive the extra reorder) and a reload (the step counter restarts, first step corrective again)."""
+    c = wl.config(4, scale=0.04)
+    p = dict(c.params, integrator=1, verlet_steps=3)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype, c.motions).step_verlet(7, 3)
+    with sph.Sph(p) as S:
+        for _ in range(2):
+            S.load_case(c)
+            S.step(3)
+            S.compute_interactions()
+            S.step(4)
+            assert S.get_info().t == pytest.approx(st.t, rel=1e-5)
+            assert np.abs(S.read_state(sph.SPH_POS) - st.pos).max() <= 1e-3 * c.params["dp"]
+            assert_close("rho", S.read_state(sph.SPH_RHO), st.rho, rtol=1e-5, floor=0)

@@ -379,6 +379,68 @@ def test_p13_density_pade_form_two_particles():
     assert np.all(st.rho > 1000.0)    # approaching particles compress
 
 
+# ---- NEXT-1: Verlet scheme (Eq. 30-31) --------------------------------------------
+def test_verlet_free_fall_closed_form():
+    # constant F = g: both Eq. 30 and Eq. 31 reproduce v0 + g t and r0 + v0 t + g t^2/2 exactly at the step times
+    p = base_params(g=(0.0, 0.0, -9.81))
+    p["domain_min"] = (-1, -1, -1); p["domain_max"] = (1, 1, 1)
+    pos = np.array([[0.1, 0.2, 0.3]]); vel = np.array([[0.3, -0.1, 0.5]], np.float32)
+    for ns in (1, 3, 40):
+        st = oracle.State(p, pos, vel, np.array([1000.0]), np.zeros(1, np.uint8))
+        x0 = st.pos.copy(); v0 = st.vel.copy()
+        st.step_verlet(7, ns)
+        t = st.t
+        g = np.array([0, 0, -9.81])
+        assert st.kstep == 7
+        assert np.allclose(st.dt_hist, 0.2 * min(math.sqrt(p["h"] / 9.81), p["h"] / p["c0"]), rtol=1e-12)
+        np.testing.assert_allclose(st.vel[0], v0[0] + g * t, rtol=1e-12)
+        q = 2 ** -22 * oracle.grid(p)[0]
+        np.testing.assert_allclose(st.pos[0], x0[0] + v0[0] * t + 0.5 * g * t * t, atol=8 * q)
+        assert st.rho[0] == 1000.0
+
+
+def test_verlet_regular_and_corrective_branches():
+    # One particle, F = g, R = 0, with a hand-set state n-1 that is NOT on the trajectory, so that the two
+    # branches give different, closed-form answers: Eq. 30 starts from (v, rho)^{n-1}, Eq. 31 from (v, rho)^n;
+    # the step counter k selects Eq. 31 when k mod N_S == 0.
+    p = base_params(g=(0.0, 0.0, -9.81))
+    p["domain_min"] = (-1, -1, -1); p["domain_max"] = (1, 1, 1)
+    g = np.array([0, 0, -9.81])
+    dt = 0.2 * min(math.sqrt(p["h"] / 9.81), p["h"] / p["c0"])
+    for k, corrective in ((0, True), (1, False), (2, False), (3, True), (6, True), (7, False)):
+        st = oracle.State(p, np.array([[0.1, 0.2, 0.3]]), np.array([[0.3, -0.1, 0.5]]), np.array([1003.0]),
+                          np.zeros(1, np.uint8))
+        st.step_verlet(0, 3)                       # creates the n-1 state and the counter
+        st.vel_m1[:] = [[-1.0, 2.0, 0.25]]; st.rho_m1[:] = [990.0]; st.kstep = k
+        x0, v0 = st.pos.copy(), st.vel.copy()
+        st.step_verlet(1, 3)
+        if corrective:
+            np.testing.assert_allclose(st.vel[0], v0[0] + dt * g, rtol=1e-13)
+            assert st.rho[0] == 1003.0
+        else:
+            np.testing.assert_allclose(st.vel[0], np.array([-1.0, 2.0, 0.25]) + 2 * dt * g, rtol=1e-13)
+            assert st.rho[0] == 990.0
+        q = 2 ** -22 * oracle.grid(p)[0]
+        np.testing.assert_allclose(st.pos[0], x0[0] + dt * v0[0] + 0.5 * dt * dt * g, atol=2 * q)
+        np.testing.assert_allclose(st.vel_m1[0], v0[0], rtol=0)      # state n becomes state n-1
+        assert st.rho_m1[0] == 1003.0 and st.kstep == k + 1
+
+
+def test_verlet_density_leapfrog_two_particles():
+    # rho^{n+1} = rho^{n-1} + 2 dt R^n with R^n from the (separately pinned) interaction pass: consistency of
+    # the update with Eq. 30, not an independent pin of R.
+    p, st = two_particles([0.5, 0.0, 0.0], rho_b=1000.0, alpha=0.0, delta=0.0)
+    st.step_verlet(1, 40)                          # first step: Eq. 31
+    r_n = st.interactions(0)
+    dt = oracle.dt(p, r_n["acc"], st.ptype, st.out, r_n["viscmax"])
+    v_n, rho_n, v_m1, rho_m1 = st.vel.copy(), st.rho.copy(), st.vel_m1.copy(), st.rho_m1.copy()
+    st.step_verlet(1, 40)                          # second step: Eq. 30
+    np.testing.assert_allclose(st.rho, rho_m1 + 2 * dt * r_n["drho"], rtol=1e-14)
+    np.testing.assert_allclose(st.vel, v_m1 + 2 * dt * r_n["acc"], rtol=1e-13, atol=1e-16)
+    np.testing.assert_allclose(st.rho_m1, rho_n, rtol=0)
+    np.testing.assert_allclose(st.vel_m1, v_n, rtol=0)
+
+
 def test_p13_second_order_convergence():
     # the predictor-corrector is second order accurate in time: halving dt (via CFL)
     # must cut the error of v by ~4x.  A dropped half step or a wrong state in the corrector gives 2x.
