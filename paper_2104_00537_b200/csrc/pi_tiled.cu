@@ -19,7 +19,7 @@ namespace {
 
 template <int DIM>
 struct TileCfg {
-  static constexpr int TX = 2, TY = DIM == 3 ? 2 : 1, TZ = 2;
+  static constexpr int TX = DIM == 3 ? 2 : 6, TY = DIM == 3 ? 2 : 1, TZ = DIM == 3 ? 2 : 6;   // 2-D: 6x6 cells per tile (swept on config 1)
   static constexpr int SX = TX + 2, SY = DIM == 3 ? TY + 2 : 1, SZ = TZ + 2;
   static constexpr int NCELL = SX * SY * SZ;   // staged cells per type block
   static constexpr int NR = 2 * NCELL;         // staged ranges: block 0 = boundary, block 1 = fluid
@@ -435,5 +435,5 @@ int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (C.k != 1) return -1;
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
   if (C.dim == 3) return launch_tiled<3, 512, 4992>(C, A, s);
-  return launch_tiled<2, 64, 1024>(C, A, s);
+  return launch_tiled<2, 128, 1024>(C, A, s);
 }
