@@ -248,12 +248,12 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   const unsigned lt_mask = (1u << r) - 1u;               // lanes of the quarter-warp below this one
 
   while (ri < nruns) {
-    // ================= T phase: fill the pools (until one of them may overflow) =================
+    // ================= T phase: fill the pools (until one of them would overflow) =================
     const int ri_end = (A_FLUID && ri < 9) ? 9 : nruns;
     const bool ddt_round = !(A_FLUID && ri < 9 && !C.ddt_over_boundary);
     int nw = 0;
     unsigned npool = 0;
-    while (ri < ri_end && !__any_sync(0xffffffffu, npool + 8 > QCAP)) {
+    while (ri < ri_end) {
       if (gw < 0) {   // open run ri
         // row ri of the stencil: cells (cx-1 .. cx+1, cy+dy, cz+dz) of one type block are one contiguous range
         const int row = ((A_FLUID && ri < 9) ? row0 - QNCELL : row0) + c_rowoff[(A_FLUID && ri >= 9) ? ri - 9 : ri];
@@ -300,6 +300,8 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       // with the byte address of the record of bit 0 (bit p -> + 256 (p & 15) + 128 (p >> 4))
       {
         const unsigned nzq = __byte_perm(__ballot_sync(0xffffffffu, u != 0u), 0u, qsel);
+        // a pool would overflow: run the P phase first; this word is recomputed in the next round (rare)
+        if (__any_sync(0xffffffffu, npool + (unsigned)__popc(nzq) > (unsigned)QCAP)) break;
         if (u != 0u)
           bmq[npool + (unsigned)__popc(nzq & lt_mask)] = make_uint2(u, ((unsigned)gw * 16u + (unsigned)r) * 16u);
         npool += (unsigned)__popc(nzq);
