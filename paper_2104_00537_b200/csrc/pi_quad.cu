@@ -442,12 +442,20 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   const int tx = tile % ntx, ty = (tile / ntx) % nty, tz = tile / (ntx * nty);
   const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
 
+  // A tile whose staged set does not fit in shared memory (compressed or crowded regions) is processed as two
+  // half tiles in z: part 1 = centre cells cz = 0 with the staged layers iz = 0..2, part 2 = cz = 1 with
+  // iz = 1..3 (the other layer counts as empty).  Only a half that still does not fit takes the global-gather path.
+  for (int part = 0; part < 3; part++) {
+  const int zlo = part == 2 ? 1 : 0, zhi = part == 1 ? 2 : 3;        // staged layers in use
+  const int czlo = part == 2 ? 1 : 0, czhi = part == 1 ? 0 : 1;      // centre layers computed
+  if (part) __syncthreads();
+
   // 1. global ranges of the staged cells (both type blocks)
   for (int rr = tid; rr < QNR; rr += NT) {
     const int blk = rr / QNCELL, c = rr % QNCELL;
     const int ix = c % QS, iy = (c / QS) % QS, iz = c / (QS * QS);
     int g[3] = {ox + ix - 1, oy + iy - 1, oz + iz - 1};
-    bool valid = true;
+    bool valid = iz >= zlo && iz <= zhi;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
       if (C.per[k]) g[k] = (g[k] + C.nc[k]) % C.nc[k];
@@ -497,7 +505,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     for (int s = 0; s < QNSEG; s++) {
       const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
       uint32_t n = 0;
-      if (cx < vx && cy < vy && cz < vz) n = s_cnt[qrange(blk, 1 + cx, 1 + cy, 1 + cz)];
+      if (cx < vx && cy < vy && cz < vz && cz >= czlo && cz <= czhi) n = s_cnt[qrange(blk, 1 + cx, 1 + cy, 1 + cz)];
       S.seg[1 + s] = run;
       run += (n + 7) / 8;
     }
@@ -506,14 +514,18 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   }
   __syncthreads();
   const uint32_t ngroups = S.seg[1 + QNSEG];
-  if (ngroups == 0) continue;                     // nothing to compute in this tile
+  if (ngroups == 0) {                             // nothing to compute in this (half) tile
+    if (part == 0) break;
+    continue;
+  }
   const uint32_t total = S.soff[QNR];
 
   if (total + 1 > (uint32_t)NMAX) {
-    // staged set does not fit in shared memory (very crowded cells): per-particle global gather
+    if (part == 0) continue;                      // retry as two half tiles
+    // even the half tile does not fit (very crowded cells): per-particle global gather
     for (int s = 0; s < QNSEG; s++) {
       const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
-      if (cx >= vx || cy >= vy || cz >= vz) continue;
+      if (cx >= vx || cy >= vy || cz >= vz || cz < czlo || cz > czhi) continue;
       const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
       const uint32_t g0 = S.gstart[rr], len = s_cnt[rr];
       for (uint32_t i = tid; i < len; i += NT) gather_one<3>(C, A, g0 + i, blk == 1, f2max, viscmax, nbsum);
@@ -578,6 +590,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     if (blk == 1) process_group<true>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
     else process_group<false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
   }
+  if (part == 0) break;
+  }   // parts
  }   // tiles
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
