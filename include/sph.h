@@ -70,6 +70,10 @@ typedef struct sph_params {
                              /*   1: Verlet, Eq. 30-31 (one pass per step)         */
   int32_t verlet_steps;      /* N_S of Eq. 31: step k is corrective when k mod N_S == 0 (the first   */
                              /*   step included); 0 -> 40 ("N_S ~ 40 is recommended")  */
+  int32_t visco_model;       /* 0: artificial viscosity, Eq. 21-22 (alpha); 1: laminar viscosity, Eq. 23  */
+                             /*   (nu0 replaces the artificial term of Eq. 22)      */
+  int32_t reserved0;         /* must be 0                                                            */
+  double nu0;                /* kinematic viscosity of Eq. 23                                        */
   sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
   sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */
   void* user;                /* passed back to dev_alloc / dev_free                                  */

@@ -26,6 +26,8 @@ class OrcParams(C.Structure):
         ("rho_bound_floor", C.c_int),
         ("cell_div", C.c_int),
         ("cell_size", C.c_double),
+        ("visco_model", C.c_int),
+        ("nu0", C.c_double),
     ]
 
 
@@ -63,6 +65,8 @@ def make_params(p: dict) -> OrcParams:
     for k in ("g", "domain_min", "domain_max"):
         getattr(s, k)[:] = [float(x) for x in p[k]]
     s.periodic[:] = [int(x) for x in p["periodic"]]
+    s.visco_model = int(p.get("visco_model", 0))
+    s.nu0 = float(p.get("nu0", 0.0))
     return s
 
 

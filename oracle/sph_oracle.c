@@ -49,6 +49,8 @@ typedef struct {
   int rho_bound_floor;    /* A10 */
   int cell_div;           /* k: cells of size 2h/k, stencil (2k+1)^dim */
   double cell_size;       /* 0 -> 2h/k */
+  int visco_model;        /* 0: artificial viscosity, Eq. 21-22; 1: laminar viscosity, Eq. 23 (NEXT-2) */
+  double nu0;             /* kinematic viscosity of Eq. 23 */
 } orc_params;
 
 typedef struct {
@@ -277,8 +279,16 @@ static inline void pair_terms(const consts_t* C, const orc_params* p, int a_flui
     double Pi = 0.0;
     if (vr < 0.0) Pi = -C->alpha * C->c0 * mu / (0.5 * (rho_a + rho_b));
     /* momentum, Eq. 22: - sum m_b ( (P_a + P_b)/(rho_a rho_b) + Pi_ab ) grad W */
+    if (p->visco_model == 1) Pi = 0.0;    /* laminar: Eq. 23 replaces the artificial term of Eq. 22 (A22) */
     double coef = -C->m * ((P_a + P_b) / (rho_a * rho_b) + Pi) * f;
     A->F[0] += coef * r[0]; A->F[1] += coef * r[1]; A->F[2] += coef * r[2];
+    if (p->visco_model == 1) {
+      /* laminar viscosity, Eq. 23 (Lo & Shao):
+       * nu0 lap(v)_a = sum_b m_b 4 nu0 (r_ab . grad_a W_ab) / ((rho_a + rho_b)(r_ab^2 + eta^2)) v_ab,
+       * with r_ab . grad_a W_ab = f r^2 */
+      double lam = C->m * 4.0 * p->nu0 * (f * r2) / ((rho_a + rho_b) * (r2 + C->eta2));
+      A->F[0] += lam * v[0]; A->F[1] += lam * v[1]; A->F[2] += lam * v[2];
+    }
   }
 }
 

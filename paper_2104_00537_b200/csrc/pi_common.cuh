@@ -32,6 +32,7 @@ struct PairAcc {
   float sc;           // sum (1/rho_b) w^3 (dv.du)                            -> continuity, Eq. 15 / 36
   float sd;           // sum_F (1/rho_b) w^3 (rho_a - rho_b)                  -> density diffusion, Eq. 17-18 (A3)
   float visc;         // max |mu_ab| / c_mu
+  float lx, ly, lz;   // sum w^3 r2u / ((r2u + eta2u)(rho_a + rho_b)) dv        -> laminar viscosity, Eq. 23
 };
 
 // One accepted ordered pair, fluid a.  DDT: include the diffusion term for this b (fluid b, or any b
@@ -58,6 +59,12 @@ __device__ __forceinline__ void pair_fluid(const DevConsts& C, float dux, float 
   A.sx = fmaf(coef, dux, A.sx);
   A.sy = fmaf(coef, duy, A.sy);
   A.sz = fmaf(coef, duz, A.sz);
+  if (C.visco_model == 1) {                      // Eq. 23 (c_pi = 0 in this model)
+    float lam = w3 * r2u * x;
+    A.lx = fmaf(lam, dvx, A.lx);
+    A.ly = fmaf(lam, dvy, A.ly);
+    A.lz = fmaf(lam, dvz, A.lz);
+  }
 }
 
 // One accepted ordered pair, boundary a <- fluid b (Eq. 36): continuity only.
@@ -79,6 +86,11 @@ __device__ __forceinline__ float4 finish_particle(const DevConsts& C, bool fluid
     r.x = fmaf(C.c_mom, A.sx, C.g[0]);
     r.y = fmaf(C.c_mom, A.sy, C.g[1]);
     r.z = fmaf(C.c_mom, A.sz, C.g[2]);
+    if (C.visco_model == 1) {
+      r.x = fmaf(C.c_lam, A.lx, r.x);
+      r.y = fmaf(C.c_lam, A.ly, r.y);
+      r.z = fmaf(C.c_lam, A.lz, r.z);
+    }
     r.w = fmaf(rho_a * C.c_cont, A.sc, C.c_ddt * A.sd);
   } else {
     r.x = r.y = r.z = 0.f;
@@ -116,7 +128,7 @@ __device__ __forceinline__ void gather_one(const DevConsts& C, const PiArgs& A, 
   ca[1] = r % C.nc[1];
   ca[2] = r / C.nc[1];
   const float inv_rho_a = fast_rcp(pa.w);
-  PairAcc S = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  PairAcc S = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   unsigned int nb = 0;
   const int K = C.k;
   const int ky = DIM == 3 ? K : 0;

@@ -124,13 +124,14 @@ struct PairAcc2 {
   f2 sx, sy, sz, sc, sd;
   float visc0, visc1;
   f2 nb;              // neighbour counts, kept as floats (exact integers)
+  f2 lx, ly, lz;      // laminar viscosity sums, Eq. 23 (LAM instantiations only)
 };
 
 // One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free.  A b outside the
 // support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record) gets weight 0:
 // w = max(1 - q/2, 0).  nb counts the exact canonical predicate C2.  pb = (x, y, z, rho_b), vb = (v_b, P_b/rho_b).
 // DDT: this b enters the density diffusion term (A4).
-template <bool A_FLUID, bool DDT>
+template <bool A_FLUID, bool DDT, bool LAM>
 __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const float4 pb, const float4 vb,
                                       PairAcc2& A) {
   const f2 dux = f2_add(a.x, f2_bc(-pb.x));   // exact (C1)
@@ -157,7 +158,14 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
     if (DDT) f2_fma_acc(gb, f2_add(a.rho, f2_bc(-pb.w)), A.sd);
     const f2 rs = f2_add(a.rho, f2_bc(pb.w));
     const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), rs);
-    const f2 y = f2_mul(dot, f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den))));   // dot / ((r2 + eta2) rs)
+    const f2 xinv = f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den)));
+    const f2 y = f2_mul(dot, xinv);                       // dot / ((r2 + eta2) rs)
+    if (LAM) {                                            // Eq. 23: sum w^3 r2u / ((r2u + eta2u) rs) dv
+      const f2 lam = f2_mul(f2_mul(w3, r2), xinv);
+      f2_fma_acc(lam, dvx, A.lx);
+      f2_fma_acc(lam, dvy, A.ly);
+      f2_fma_acc(lam, dvz, A.lz);
+    }
     const f2 mu = f2_mul(y, rs);                          // mu_ab / c_mu   (Eq. 21, A12)
     A.visc0 = fmaxf(A.visc0, fabsf(f2_lo(mu)));
     A.visc1 = fmaxf(A.visc1, fabsf(f2_hi(mu)));
@@ -199,7 +207,7 @@ __device__ __forceinline__ unsigned qsumu(unsigned v) {
 
 // One a-group: up to 8 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
 // A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw is this warp's pool area ([4][QCAP] uint2).
-template <bool A_FLUID>
+template <bool A_FLUID, bool LAM>
 __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint2* bmw, int cx,
                                               int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp,
                                               unsigned total, float& f2max, float& viscmax, unsigned int& nbsum) {
@@ -231,7 +239,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     nz1 = __float2half2_rn(act1 ? -2.f * p1.z : 0.f); th1 = __half2half2(__float2half_ru(thr1));
   }
   PairAcc2 acc;
-  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = acc.nb = f2_pack(0.f, 0.f);
+  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = acc.nb = acc.lx = acc.ly = acc.lz = f2_pack(0.f, 0.f);
   acc.visc0 = acc.visc1 = 0.f;
 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
@@ -349,9 +357,9 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     Q_FETCH(pbA, vbA)                                                                                  \
     while (more) { /* single exit: at most one surplus evaluation of dummy records per round */        \
       Q_FETCH(pbB, vbB)                                                                                \
-      pair2<A_FLUID, DDT>(C, a, pbA, vbA, acc);                                                        \
+      pair2<A_FLUID, DDT, LAM>(C, a, pbA, vbA, acc);                                                        \
       Q_FETCH(pbA, vbA)                                                                                \
-      pair2<A_FLUID, DDT>(C, a, pbB, vbB, acc);                                                        \
+      pair2<A_FLUID, DDT, LAM>(C, a, pbB, vbB, acc);                                                        \
     }                                                                                                  \
   }
     if (ddt_round) Q_LOOP(true) else Q_LOOP(false)
@@ -370,6 +378,11 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     r0.sz = qsum(f2_lo(acc.sz)); r1.sz = qsum(f2_hi(acc.sz));
     r0.sd = qsum(f2_lo(acc.sd)); r1.sd = qsum(f2_hi(acc.sd));
     r0.visc = qmax(acc.visc0); r1.visc = qmax(acc.visc1);
+    if (LAM) {
+      r0.lx = qsum(f2_lo(acc.lx)); r1.lx = qsum(f2_hi(acc.lx));
+      r0.ly = qsum(f2_lo(acc.ly)); r1.ly = qsum(f2_hi(acc.ly));
+      r0.lz = qsum(f2_lo(acc.lz)); r1.lz = qsum(f2_hi(acc.lz));
+    }
   }
   if (r == 0) {
     const int ra = qrange(A_FLUID ? 1 : 0, 1 + cx, 1 + cy, 1 + cz);
@@ -413,7 +426,7 @@ __global__ void __launch_bounds__(256) k_quad_tiles(DevConsts C, const uint32_t*
 }
 
 // Persistent kernel: one CTA per SM takes active tiles from the list until it is used up.
-template <int NT, int NMAX>
+template <int NT, int NMAX, bool LAM>
 __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int ntx, int nty) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NWARP = NT / 32;
@@ -587,8 +600,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
     const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
     const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
-    if (blk == 1) process_group<true>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
-    else process_group<false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    if (blk == 1) process_group<true, LAM>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    else process_group<false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
   }
   if (part == 0) break;
   }   // parts
@@ -596,7 +609,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
 
-template <int NT, int NMAX>
+template <int NT, int NMAX, bool LAM>
 int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
   constexpr int NWARP = NT / 32;
@@ -604,7 +617,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
                       sizeof(uint2) * NWARP * 4 * QCAP + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
   static bool configured = false;
   if (!configured) {
-    if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+    if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
         cudaSuccess) {
       cudaGetLastError();
       return -1;
@@ -625,7 +638,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   }
   if (cudaMemsetAsync(A.tile_ws, 0, 4 * sizeof(uint32_t), s) != cudaSuccess) return -1;
   k_quad_tiles<<<(unsigned)((ntiles + 255) / 256), 256, 0, s>>>(C, A.cellstart, ntx, nty, (int)ntiles, A.tile_ws);
-  k_pi_quad<NT, NMAX><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
+  k_pi_quad<NT, NMAX, LAM><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
   return 0;
 }
 
@@ -642,5 +655,6 @@ int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.dim != 3 || C.k != 1) return -1;
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
-  return launch_quad<512, 4928>(C, A, s);
+  if (C.visco_model == 1) return launch_quad<512, 4928, true>(C, A, s);   // laminar viscosity, Eq. 23
+  return launch_quad<512, 4928, false>(C, A, s);
 }

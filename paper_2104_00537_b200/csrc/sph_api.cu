@@ -158,6 +158,8 @@ int validate(const sph_params* p, std::string& why) {
   if (p->pi_kernel < 0 || p->pi_kernel > 3) return bad("pi_kernel must be 0, 1, 2 or 3");
   if (p->integrator < 0 || p->integrator > 1) return bad("integrator must be 0 (symplectic) or 1 (Verlet)");
   if (p->verlet_steps < 0) return bad("verlet_steps must be >= 0");
+  if (p->visco_model < 0 || p->visco_model > 1) return bad("visco_model must be 0 (artificial) or 1 (laminar)");
+  if (p->nu0 < 0) return bad("nu0 must be >= 0");
   const double cs_min = 2.0 * p->h / p->cell_div;
   if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
   for (int k = 0; k < 3; k++) {
@@ -213,6 +215,9 @@ int derive(const sph_params* p, DevConsts& C, std::string& why) {
   C.c_mu = (float)(p->h / cs);
   C.ddt_over_boundary = p->ddt_over_boundary;
   C.rho_bound_floor = p->rho_bound_floor;
+  C.visco_model = p->visco_model;
+  C.c_lam = (float)(4.0 * m * p->nu0 * Cf);
+  if (p->visco_model == 1) C.c_pi = 0.f;          // Eq. 23 replaces the artificial term of Eq. 22
   C.h = p->h;
   C.c0 = p->c0;
   C.cfl = p->cfl;

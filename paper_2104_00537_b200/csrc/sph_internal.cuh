@@ -25,6 +25,8 @@ struct DevConsts {
   float c_pi;              // -alpha c0 * 2 * (h/cs) : Pi_ab  = c_pi * min(dv.du,0) / ((r2u+eta2u)(rho_a+rho_b))
   float c_mu;              // h/cs                   : mu_ab  = c_mu * (dv.du) / (r2u + eta2u)
   int ddt_over_boundary, rho_bound_floor;
+  int visco_model;         // 0 artificial (Eq. 21-22), 1 laminar (Eq. 23)
+  float c_lam;             // 4 m nu0 Cf             : F_lam = c_lam * sum w^3 r2u / ((r2u+eta2u)(rho_a+rho_b)) dv
   double cs, dmin[3];
   double h, c0, cfl;
   float inv_cs;            // 1/cs (update kernel: du = dt * v / cs)

@@ -45,6 +45,9 @@ class SphParams(C.Structure):
         ("count_neighbours", C.c_int32),
         ("integrator", C.c_int32),
         ("verlet_steps", C.c_int32),
+        ("visco_model", C.c_int32),
+        ("reserved0", C.c_int32),
+        ("nu0", C.c_double),
         ("dev_alloc", ALLOC_FN),
         ("dev_free", FREE_FN),
         ("user", C.c_void_p),
@@ -139,6 +142,8 @@ class Sph:
         sp.count_neighbours = int(bool(count_neighbours))
         sp.integrator = int(params.get("integrator", 0))
         sp.verlet_steps = int(params.get("verlet_steps", 0))
+        sp.visco_model = int(params.get("visco_model", 0))
+        sp.nu0 = float(params.get("nu0", 0.0))
         self._stream = stream if stream is not None else torch.cuda.current_stream()
         sp.cuda_stream = self._stream.cuda_stream
 

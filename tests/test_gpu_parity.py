@@ -376,3 +376,33 @@ def test_verlet_moving_boundary_and_reload(sph):
             assert S.get_info().t == pytest.approx(st.t, rel=1e-5)
             assert np.abs(S.read_state(sph.SPH_POS) - st.pos).max() <= 1e-3 * c.params["dp"]
             assert_close("rho", S.read_state(sph.SPH_RHO), st.rho, rtol=1e-5, floor=0)
+
+
+# ---- NEXT-2: laminar viscosity, Eq. 23 -----------------------------------------------------
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_laminar_viscosity_one_pass(sph, pi_kernel):
+    """visco_model = 1: Eq. 23 replaces the artificial term of Eq. 22.  nu0 is chosen large enough for the
+    viscous force to matter next to the pressure force (so that a wrong term cannot hide in the tolerance)."""
+    c = developed_state(wl.config(0), 3)
+    c.params.update(visco_model=1, nu0=5.0e-3)
+    ref = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).interactions()
+    ref0 = oracle.State(dict(c.params, nu0=0.0), c.pos, c.vel, c.rho, c.ptype).interactions()
+    fl = c.ptype == 0
+    assert np.abs(ref["acc"][fl] - ref0["acc"][fl]).max() > 1e-3 * np.abs(ref["acc"][fl]).max()
+    check_one_pass(sph, c, pi_kernel)
+
+
+def test_laminar_viscosity_steps_and_2d(sph):
+    c = wl.config(0)
+    c.params.update(visco_model=1, nu0=1.0e-3)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).step(6)
+    with sph.Sph(c.params) as S:
+        S.load_case(c)
+        S.step(6)
+        assert S.get_info().pi_kernel == 3
+        assert np.abs(S.read_state(sph.SPH_POS) - st.pos).max() <= 1e-3 * c.params["dp"]
+        assert_close("rho", S.read_state(sph.SPH_RHO), st.rho, rtol=1e-5, floor=0)
+    c2 = developed_state(wl.config(1, scale=0.05), 4)      # 2-D: tiled kernel hands the laminar model to the gather kernel
+    c2.params.update(visco_model=1, nu0=1.0e-3)
+    info = check_one_pass(sph, c2, 0)
+    assert info.pi_kernel == 1

@@ -193,6 +193,35 @@ def test_p7_diffusion_is_diffusive():
     assert st2.interactions()["drho"][centre] > 0
 
 
+# ---- NEXT-2: laminar viscosity (Eq. 23) --------------------------------------------
+def test_laminar_viscosity_matches_analytic_laplacian():
+    # v_x = A y^2 + B z on a full-support lattice of uniform density: Eq. 23 -> nu0 lap(v) = (2 A nu0, 0, 0);
+    # the pressure term vanishes by symmetry (uniform rho) and the artificial term is switched off.
+    n = 17
+    c = wl.dam_break("blk", 3, DP, (n, n, n), (n, n, n), 0.0, 1, 0.3)
+    pos = c.pos[c.ptype == 0]
+    A, B, nu0 = 30.0, 0.7, 1.0e-3
+    y0 = pos[:, 1].mean()
+    vel = np.zeros_like(pos)
+    vel[:, 0] = A * (pos[:, 1] - y0) ** 2 + B * pos[:, 2]
+    rho = np.full(len(pos), 1000.0)
+    typ = np.zeros(len(pos), np.uint8)
+    p = dict(c.params, g=(0, 0, 0), visco_model=1, nu0=nu0)
+    r1 = oracle.State(p, pos, vel, rho, typ).interactions()
+    centre = np.argmin(((pos - pos.mean(0)) ** 2).sum(1))
+    assert r1["nbcount"][centre] == 304
+    assert r1["acc"][centre, 0] == pytest.approx(2 * A * nu0, rel=0.03)
+    assert abs(r1["acc"][centre, 1]) < 1e-3 * 2 * A * nu0 and abs(r1["acc"][centre, 2]) < 1e-3 * 2 * A * nu0
+    # linear in nu0, zero for nu0 = 0, and the artificial term (alpha) plays no role in this model
+    r2 = oracle.State(dict(p, nu0=2 * nu0, alpha=0.5), pos, vel, rho, typ).interactions()
+    r0 = oracle.State(dict(p, nu0=0.0), pos, vel, rho, typ).interactions()
+    np.testing.assert_allclose(r2["acc"][centre], 2 * r1["acc"][centre], rtol=1e-9, atol=1e-12)
+    assert np.abs(r0["acc"][centre]).max() < 1e-9
+    # pairwise antisymmetric: no net momentum from the viscous term (fluid only, no boundaries)
+    tot = (r1["acc"] * 1.0).sum(0)
+    assert np.abs(tot).max() < 1e-9 * np.abs(r1["acc"]).sum()
+
+
 # ---- P8: continuity against Eq. 12 (drho/dt = -rho div v) ---------------------------------------
 def test_p8_continuity_linear_velocity_field():
     n = 15
