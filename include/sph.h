@@ -72,7 +72,8 @@ typedef struct sph_params {
                              /*   step included); 0 -> 40 ("N_S ~ 40 is recommended")  */
   int32_t visco_model;       /* 0: artificial viscosity, Eq. 21-22 (alpha); 1: laminar viscosity, Eq. 23  */
                              /*   (nu0 replaces the artificial term of Eq. 22)      */
-  int32_t reserved0;         /* must be 0                                                            */
+  int32_t ddt_model;         /* density diffusion term: 0 Molteni-Colagrossi, Eq. 18; 1 Fourtakas et al.,   */
+                             /*   Eq. 19-20 (only the dynamic part of the density difference diffuses, A23) */
   double nu0;                /* kinematic viscosity of Eq. 23                                        */
   sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
   sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */

@@ -28,6 +28,7 @@ class OrcParams(C.Structure):
         ("cell_size", C.c_double),
         ("visco_model", C.c_int),
         ("nu0", C.c_double),
+        ("ddt_model", C.c_int),
     ]
 
 
@@ -67,6 +68,7 @@ def make_params(p: dict) -> OrcParams:
     s.periodic[:] = [int(x) for x in p["periodic"]]
     s.visco_model = int(p.get("visco_model", 0))
     s.nu0 = float(p.get("nu0", 0.0))
+    s.ddt_model = int(p.get("ddt_model", 0))
     return s
 
 

@@ -51,6 +51,7 @@ typedef struct {
   double cell_size;       /* 0 -> 2h/k */
   int visco_model;        /* 0: artificial viscosity, Eq. 21-22; 1: laminar viscosity, Eq. 23 (NEXT-2) */
   double nu0;             /* kinematic viscosity of Eq. 23 */
+  int ddt_model;          /* 0: Molteni-Colagrossi, Eq. 18; 1: Fourtakas et al., Eq. 19-20 (NEXT-2) */
 } orc_params;
 
 typedef struct {
@@ -266,8 +267,19 @@ static inline void pair_terms(const consts_t* C, const orc_params* p, int a_flui
 
   /* density diffusion, Eq. 17-18, diffusive reading A3: D_a = 2 delta h c0 sum (rho_a - rho_b) f V_b,
    * fluid a only, fluid b only unless ddt_over_boundary (A4); c_a = c0 (A5). */
-  if (a_fluid && (b_fluid || p->ddt_over_boundary))
-    A->R += 2.0 * C->delta * C->h * C->c0 * (rho_a - rho_b) * f * Vb;
+  if (a_fluid && (b_fluid || p->ddt_over_boundary)) {
+    double drho = rho_a - rho_b;
+    if (p->ddt_model == 1) {
+      /* Fourtakas et al., Eq. 19-20: only the dynamic part of the density difference
+       * diffuses.  The hydrostatic part is built locally from P^H_ab = rho0 g z_ab (Eq. 20; written here as
+       * rho0 g . r_ab for any direction of g) through the inverse of the Tait EOS (Eq. 28, "barotropic"):
+       * rho^H_ab = rho0 [ (1 + P^H_ab / B)^(1/gamma) - 1 ]  (reading A23). */
+      double PH = C->rho0 * (p->g[0] * r[0] + p->g[1] * r[1] + p->g[2] * r[2]);
+      double rhoH = C->rho0 * (pow(1.0 + PH / C->B, 1.0 / C->gamma) - 1.0);
+      drho -= rhoH;
+    }
+    A->R += 2.0 * C->delta * C->h * C->c0 * drho * f * Vb;
+  }
 
   /* mu_ab = h v_ab.r_ab / (r^2 + eta^2)  (Eq. 21; A12 for the dt) */
   double mu = C->h * vr / (r2 + C->eta2);

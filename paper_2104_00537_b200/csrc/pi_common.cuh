@@ -26,6 +26,15 @@ __device__ __forceinline__ float pair_r2u(float dux, float duy, float duz) {
   return __fmaf_rn(duz, duz, r2);
 }
 
+// Fourtakas DDT, Eq. 19-20 (A23): hydrostatic density difference rho^H_ab = rho0 [(1 + e)^(1/gamma) - 1] with
+// e = P^H_ab / B = rho0 g.r_ab / B.  For |e| <= 0.02 the binomial series to e^4 is exact to fp32 rounding
+// (and avoids the cancellation of forming 1 + e); otherwise expm1(log1p(e) / gamma).
+__device__ __forceinline__ float hydrostatic_drho(const DevConsts& C, float dux, float duy, float duz) {
+  const float e = fmaf(C.c_hyd[2], duz, fmaf(C.c_hyd[1], duy, C.c_hyd[0] * dux));
+  if (C.hyd_series_ok) return e * fmaf(e, fmaf(e, fmaf(e, C.hyd_k[3], C.hyd_k[2]), C.hyd_k[1]), C.hyd_k[0]);
+  return C.rho0 * expm1f(log1pf(e) * C.inv_gamma);
+}
+
 // Raw sums accumulated for one particle a.
 struct PairAcc {
   float sx, sy, sz;   // sum w^3 [(Pa+Pb)/(rho_a rho_b) + Pi_ab] du          -> momentum, Eq. 22
@@ -49,7 +58,11 @@ __device__ __forceinline__ void pair_fluid(const DevConsts& C, float dux, float 
   float dot = fmaf(dvz, duz, fmaf(dvy, duy, dvx * dux));       // v_ab . r_ab / cs
   float gb = w3 * inv_rho_b;
   A.sc = fmaf(gb, dot, A.sc);
-  if (DDT) A.sd = fmaf(gb, rho_a - pb.w, A.sd);
+  if (DDT) {
+    float drho = rho_a - pb.w;
+    if (C.ddt_model == 1) drho -= hydrostatic_drho(C, dux, duy, duz);   // Eq. 19-20
+    A.sd = fmaf(gb, drho, A.sd);
+  }
   float rs = rho_a + pb.w;
   float x = fast_rcp((r2u + C.eta2u) * rs);
   float mu = fabsf(dot) * x * rs;                // |mu_ab| / c_mu   (Eq. 21, A12)

@@ -655,6 +655,7 @@ int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.dim != 3 || C.k != 1) return -1;
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
+  if (C.ddt_model != 0) return -1;   // Fourtakas DDT (Eq. 19-20): gather kernel for now
   if (C.visco_model == 1) return launch_quad<512, 4928, true>(C, A, s);   // laminar viscosity, Eq. 23
   return launch_quad<512, 4928, false>(C, A, s);
 }

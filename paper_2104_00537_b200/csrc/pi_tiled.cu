@@ -433,7 +433,7 @@ int launch_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
 int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.k != 1) return -1;
-  if (C.visco_model != 0) return -1;   // laminar viscosity (Eq. 23): quad (3-D) or gather kernel
+  if (C.visco_model != 0 || C.ddt_model != 0) return -1;   // Eq. 23 / Eq. 19-20: quad (3-D) or gather kernel
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
   if (C.dim == 3) return launch_tiled<3, 512, 4992>(C, A, s);
   return launch_tiled<2, 128, 1024>(C, A, s);

@@ -160,6 +160,7 @@ int validate(const sph_params* p, std::string& why) {
   if (p->verlet_steps < 0) return bad("verlet_steps must be >= 0");
   if (p->visco_model < 0 || p->visco_model > 1) return bad("visco_model must be 0 (artificial) or 1 (laminar)");
   if (p->nu0 < 0) return bad("nu0 must be >= 0");
+  if (p->ddt_model < 0 || p->ddt_model > 1) return bad("ddt_model must be 0 (Molteni) or 1 (Fourtakas)");
   const double cs_min = 2.0 * p->h / p->cell_div;
   if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
   for (int k = 0; k < 3; k++) {
@@ -215,6 +216,19 @@ int derive(const sph_params* p, DevConsts& C, std::string& why) {
   C.c_mu = (float)(p->h / cs);
   C.ddt_over_boundary = p->ddt_over_boundary;
   C.rho_bound_floor = p->rho_bound_floor;
+  C.ddt_model = p->ddt_model;
+  {
+    // Fourtakas DDT (Eq. 19-20, A23): rho^H_ab = rho0 [(1 + e)^(1/gamma) - 1], e = rho0 g.r_ab / B, |r_ab| < 2h
+    const double B = p->c0 * p->c0 * p->rho0 / p->gamma, a = 1.0 / p->gamma;
+    double gn = 0.0;
+    for (int k = 0; k < 3; k++) { C.c_hyd[k] = (float)(p->rho0 * cs * p->g[k] / B); gn += p->g[k] * p->g[k]; }
+    C.hyd_series_ok = p->rho0 * sqrt(gn) * 2.0 * p->h / B <= 0.02;
+    C.hyd_k[0] = (float)(p->rho0 * a);
+    C.hyd_k[1] = (float)(p->rho0 * a * (a - 1.0) / 2.0);
+    C.hyd_k[2] = (float)(p->rho0 * a * (a - 1.0) * (a - 2.0) / 6.0);
+    C.hyd_k[3] = (float)(p->rho0 * a * (a - 1.0) * (a - 2.0) * (a - 3.0) / 24.0);
+    C.inv_gamma = (float)a;
+  }
   C.visco_model = p->visco_model;
   C.c_lam = (float)(4.0 * m * p->nu0 * Cf);
   if (p->visco_model == 1) C.c_pi = 0.f;          // Eq. 23 replaces the artificial term of Eq. 22

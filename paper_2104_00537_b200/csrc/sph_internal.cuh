@@ -26,6 +26,11 @@ struct DevConsts {
   float c_mu;              // h/cs                   : mu_ab  = c_mu * (dv.du) / (r2u + eta2u)
   int ddt_over_boundary, rho_bound_floor;
   int visco_model;         // 0 artificial (Eq. 21-22), 1 laminar (Eq. 23)
+  int ddt_model;           // 0 Molteni (Eq. 18), 1 Fourtakas (Eq. 19-20)
+  int hyd_series_ok;       // |e| <= 0.02 for every pair: the binomial series below is exact to fp32 rounding
+  float c_hyd[3];          // e = P^H_ab / B = sum_k c_hyd[k] du_k,  c_hyd[k] = rho0 cs g_k / B   (Eq. 20)
+  float hyd_k[4];          // rho^H_ab = e (k0 + e (k1 + e (k2 + e k3))) = rho0 [(1 + e)^(1/gamma) - 1]
+  float inv_gamma;
   float c_lam;             // 4 m nu0 Cf             : F_lam = c_lam * sum w^3 r2u / ((r2u+eta2u)(rho_a+rho_b)) dv
   double cs, dmin[3];
   double h, c0, cfl;

@@ -46,7 +46,7 @@ class SphParams(C.Structure):
         ("integrator", C.c_int32),
         ("verlet_steps", C.c_int32),
         ("visco_model", C.c_int32),
-        ("reserved0", C.c_int32),
+        ("ddt_model", C.c_int32),
         ("nu0", C.c_double),
         ("dev_alloc", ALLOC_FN),
         ("dev_free", FREE_FN),
@@ -144,6 +144,7 @@ class Sph:
         sp.verlet_steps = int(params.get("verlet_steps", 0))
         sp.visco_model = int(params.get("visco_model", 0))
         sp.nu0 = float(params.get("nu0", 0.0))
+        sp.ddt_model = int(params.get("ddt_model", 0))
         self._stream = stream if stream is not None else torch.cuda.current_stream()
         sp.cuda_stream = self._stream.cuda_stream
 

@@ -406,3 +406,34 @@ def test_laminar_viscosity_steps_and_2d(sph):
     c2.params.update(visco_model=1, nu0=1.0e-3)
     info = check_one_pass(sph, c2, 0)
     assert info.pi_kernel == 1
+
+
+# ---- NEXT-2: Fourtakas density diffusion, Eq. 19-20 ----------------------------------------
+@pytest.mark.parametrize("case_name", ["dam_break", "column"])
+def test_fourtakas_ddt_one_pass(sph, case_name):
+    """ddt_model = 1: only the dynamic part of the density difference diffuses (A23).  The resting column with
+    hydrostatic density is the case the term was made for: drho/dt there is dominated by the diffusion term."""
+    if case_name == "dam_break":
+        c = developed_state(wl.config(0), 3)
+    else:
+        c = wl.hydrostatic_column("col", 0.02, (10, 10, 24), 20)
+    c.params.update(ddt_model=1, delta=0.1)
+    ref = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).interactions()
+    ref0 = oracle.State(dict(c.params, ddt_model=0), c.pos, c.vel, c.rho, c.ptype).interactions()
+    assert np.abs(ref["drho"] - ref0["drho"]).max() > 1e-2 * np.abs(ref0["drho"]).max()   # the model matters here
+    if case_name == "dam_break":
+        info = check_one_pass(sph, c, 0)
+        assert info.pi_kernel == 1
+        return
+    # Resting column: the acceleration is the small difference of the pressure force and gravity (|F_a| ~ 0.3 of
+    # |g| = 9.81), so it is compared relative to the pressure force it is made of; drho/dt keeps the stated tolerance.
+    with sph.Sph(c.params, count_neighbours=True) as S:
+        S.load_case(c)
+        S.compute_interactions()
+        act = ref["nbcount"] >= 0
+        assert np.array_equal(S.read_state(sph.SPH_NBCOUNT), ref["nbcount"])
+        assert_close("drho", S.read_state(sph.SPH_DRHODT)[act], ref["drho"][act])
+        g = np.array(c.params["g"])
+        fl = c.ptype == 0
+        assert_close("pressure force", S.read_state(sph.SPH_ACC)[fl] - g, ref["acc"][fl] - g, rtol=1e-4, floor=1e-5)
+        assert S.get_info().pi_kernel == 1

@@ -222,6 +222,51 @@ def test_laminar_viscosity_matches_analytic_laplacian():
     assert np.abs(tot).max() < 1e-9 * np.abs(r1["acc"]).sum()
 
 
+# ---- NEXT-2: Fourtakas density diffusion (Eq. 19-20) -------------------------------
+def test_fourtakas_ddt_removes_the_hydrostatic_gradient_and_reduces_to_molteni_without_gravity():
+    # Resting column with the hydrostatic density profile (fluid only, no walls).
+    c = wl.hydrostatic_column("col", DP, (12, 12, 30), 26)
+    fl = c.ptype == 0
+    pos, rho = c.pos[fl], c.rho[fl].astype(np.float64)
+    typ = np.zeros(len(pos), np.uint8); vel = np.zeros_like(pos)
+    def D(params):
+        r1 = oracle.State(params, pos, vel, rho, typ).interactions()
+        r0 = oracle.State(dict(params, delta=0.0), pos, vel, rho, typ).interactions()
+        return r1["drho"] - r0["drho"], r1["nbcount"]
+    p = dict(c.params)
+    Dm, nb = D(dict(p, ddt_model=0))
+    Df, _ = D(dict(p, ddt_model=1))
+    inner = nb == 304                                    # full kernel support
+    assert inner.sum() > 50
+    # Truncated support (top and bottom layer of the fluid block): Eq. 18 sees the whole hydrostatic density
+    # gradient, Eq. 19-20 removes it pair by pair ("improves the behaviour of pressure near the wall boundaries").
+    z = pos[:, 2]
+    for layer in (z.max(), z.min()):
+        m = np.isclose(z, layer) & (nb == nb[np.isclose(z, layer)].max())
+        assert m.sum() > 10
+        assert np.abs(Dm[m]).min() > 30.0
+        assert np.abs(Df[m]).max() < 0.1 * np.abs(Dm[m]).min()
+    # Full support: the odd (gradient) part cancels by symmetry in both models; what is left is the curvature of
+    # the hydrostatic profile, two orders of magnitude below the truncated-support values.
+    assert np.abs(Dm[inner]).max() < 1.0 and np.abs(Df[inner]).max() < 1.0
+    # a dynamic density bump on top of the hydrostatic profile diffuses like Eq. 18 does without gravity
+    centre = np.argmin(((pos - pos[inner].mean(0)) ** 2).sum(1))
+    rho_b = rho.copy(); rho_b[centre] += 2.0
+    def D1(params, rr):
+        r1 = oracle.State(params, pos, vel, rr, typ).interactions()
+        r0 = oracle.State(dict(params, delta=0.0), pos, vel, rr, typ).interactions()
+        return (r1["drho"] - r0["drho"])[centre]
+    bump_f = D1(dict(p, ddt_model=1), rho_b) - D1(dict(p, ddt_model=1), rho)
+    flat = np.full(len(pos), 1000.0); flat_b = flat.copy(); flat_b[centre] += 2.0
+    bump_m = D1(dict(p, ddt_model=0, g=(0, 0, 0)), flat_b)
+    assert bump_f < 0 and bump_f == pytest.approx(bump_m, rel=2e-2)
+    # without gravity the two models coincide exactly
+    rr = 1000.0 + 3.0 * np.sin(40 * pos[:, 0])
+    a = oracle.State(dict(p, g=(0, 0, 0), ddt_model=1), pos, vel, rr, typ).interactions()["drho"]
+    b = oracle.State(dict(p, g=(0, 0, 0), ddt_model=0), pos, vel, rr, typ).interactions()["drho"]
+    np.testing.assert_allclose(a, b, rtol=1e-13, atol=1e-13)
+
+
 # ---- P8: continuity against Eq. 12 (drho/dt = -rho div v) ---------------------------------------
 def test_p8_continuity_linear_velocity_field():
     n = 15
