@@ -131,7 +131,7 @@ struct PairAcc2 {
 // support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record) gets weight 0:
 // w = max(1 - q/2, 0).  nb counts the exact canonical predicate C2.  pb = (x, y, z, rho_b), vb = (v_b, P_b/rho_b).
 // DDT: this b enters the density diffusion term (A4).
-template <bool A_FLUID, bool DDT, bool LAM>
+template <bool A_FLUID, bool DDT, bool LAM, bool FOURT>
 __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const float4 pb, const float4 vb,
                                       PairAcc2& A) {
   const f2 dux = f2_add(a.x, f2_bc(-pb.x));   // exact (C1)
@@ -155,7 +155,19 @@ __device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const 
   const f2 gb = f2_mul(w3, f2_bc(inv_rho_b));
   f2_fma_acc(gb, dot, A.sc);
   if (A_FLUID) {
-    if (DDT) f2_fma_acc(gb, f2_add(a.rho, f2_bc(-pb.w)), A.sd);
+    if (DDT) {
+      f2 drho = f2_add(a.rho, f2_bc(-pb.w));
+      if (FOURT) {   // Eq. 19-20 (A23): minus rho^H_ab = e (k0 + e (k1 + e (k2 + e k3))), e = c_hyd . du
+        f2 e = f2_mul(dux, f2_bc(C.c_hyd[0]));
+        e = f2_fma(duy, f2_bc(C.c_hyd[1]), e);
+        e = f2_fma(duz, f2_bc(C.c_hyd[2]), e);
+        f2 h = f2_fma(e, f2_bc(C.hyd_k[3]), f2_bc(C.hyd_k[2]));
+        h = f2_fma(e, h, f2_bc(C.hyd_k[1]));
+        h = f2_fma(e, h, f2_bc(C.hyd_k[0]));
+        drho = f2_fma(f2_mul(e, f2_bc(-1.0f)), h, drho);
+      }
+      f2_fma_acc(gb, drho, A.sd);
+    }
     const f2 rs = f2_add(a.rho, f2_bc(pb.w));
     const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), rs);
     const f2 xinv = f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den)));
@@ -207,7 +219,7 @@ __device__ __forceinline__ unsigned qsumu(unsigned v) {
 
 // One a-group: up to 8 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
 // A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw is this warp's pool area ([4][QCAP] uint2).
-template <bool A_FLUID, bool LAM>
+template <bool A_FLUID, bool LAM, bool FOURT>
 __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint2* bmw, int cx,
                                               int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp,
                                               unsigned total, float& f2max, float& viscmax, unsigned int& nbsum) {
@@ -357,9 +369,9 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     Q_FETCH(pbA, vbA)                                                                                  \
     while (more) { /* single exit: at most one surplus evaluation of dummy records per round */        \
       Q_FETCH(pbB, vbB)                                                                                \
-      pair2<A_FLUID, DDT, LAM>(C, a, pbA, vbA, acc);                                                        \
+      pair2<A_FLUID, DDT, LAM, FOURT>(C, a, pbA, vbA, acc);                                                        \
       Q_FETCH(pbA, vbA)                                                                                \
-      pair2<A_FLUID, DDT, LAM>(C, a, pbB, vbB, acc);                                                        \
+      pair2<A_FLUID, DDT, LAM, FOURT>(C, a, pbB, vbB, acc);                                                        \
     }                                                                                                  \
   }
     if (ddt_round) Q_LOOP(true) else Q_LOOP(false)
@@ -426,7 +438,7 @@ __global__ void __launch_bounds__(256) k_quad_tiles(DevConsts C, const uint32_t*
 }
 
 // Persistent kernel: one CTA per SM takes active tiles from the list until it is used up.
-template <int NT, int NMAX, bool LAM>
+template <int NT, int NMAX, bool LAM, bool FOURT>
 __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int ntx, int nty) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NWARP = NT / 32;
@@ -600,8 +612,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
     const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
     const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
-    if (blk == 1) process_group<true, LAM>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
-    else process_group<false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    if (blk == 1) process_group<true, LAM, FOURT>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    else process_group<false, false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
   }
   if (part == 0) break;
   }   // parts
@@ -609,7 +621,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
 
-template <int NT, int NMAX, bool LAM>
+template <int NT, int NMAX, bool LAM, bool FOURT>
 int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
   constexpr int NWARP = NT / 32;
@@ -617,7 +629,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
                       sizeof(uint2) * NWARP * 4 * QCAP + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
   static bool configured = false;
   if (!configured) {
-    if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+    if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM, FOURT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
         cudaSuccess) {
       cudaGetLastError();
       return -1;
@@ -638,7 +650,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   }
   if (cudaMemsetAsync(A.tile_ws, 0, 4 * sizeof(uint32_t), s) != cudaSuccess) return -1;
   k_quad_tiles<<<(unsigned)((ntiles + 255) / 256), 256, 0, s>>>(C, A.cellstart, ntx, nty, (int)ntiles, A.tile_ws);
-  k_pi_quad<NT, NMAX, LAM><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
+  k_pi_quad<NT, NMAX, LAM, FOURT><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
   return 0;
 }
 
@@ -655,7 +667,11 @@ int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.dim != 3 || C.k != 1) return -1;
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
-  if (C.ddt_model != 0) return -1;   // Fourtakas DDT (Eq. 19-20): gather kernel for now
-  if (C.visco_model == 1) return launch_quad<512, 4928, true>(C, A, s);   // laminar viscosity, Eq. 23
-  return launch_quad<512, 4928, false>(C, A, s);
+  // the packed Fourtakas term uses the series form of the inverse EOS (exact to fp32 rounding for |e| <= 0.02)
+  if (C.ddt_model == 1 && !C.hyd_series_ok) return -1;
+  const bool lam = C.visco_model == 1, fourt = C.ddt_model == 1;   // Eq. 23 / Eq. 19-20 instantiations
+  if (lam && fourt) return launch_quad<512, 4928, true, true>(C, A, s);
+  if (lam) return launch_quad<512, 4928, true, false>(C, A, s);
+  if (fourt) return launch_quad<512, 4928, false, true>(C, A, s);
+  return launch_quad<512, 4928, false, false>(C, A, s);
 }
