@@ -161,6 +161,20 @@ def test_config2_full_size_bench_configuration(sph):
     assert info.n_interactions > 1_200_000_000
 
 
+def test_config3_full_size_periodic_cloud(sph):
+    """BASELINE.json configs[3] at full size (16.0 M particles in a fully periodic cube, jitter 0.2 dp, seeded
+    velocities and densities): every particle against the oracle, plus the size-independent invariants P5/P6
+    (no net momentum change without gravity and boundaries; the diffusion term conserves mass)."""
+    c = wl.config(3)
+    info = check_one_pass(sph, c, 0)
+    assert info.pi_kernel == 3 and info.n == 16003008
+    with sph.Sph(c.params) as S:
+        S.load_case(c)
+        S.compute_interactions()
+        acc = S.read_state(sph.SPH_ACC).astype(np.float64)
+        assert np.abs(acc.sum(0)).max() <= 1e-6 * np.abs(acc).sum(0).max()
+
+
 @pytest.mark.parametrize("pi_kernel", KERNELS)
 def test_borderline_shells(sph, pi_kernel):
     """Neighbour counts stay bit exact when many pairs sit within 1e-3 .. 1e-6 of the support radius, with the
