@@ -3,7 +3,7 @@
  * hot path of weakly compressible SPH (arxiv 2104.00537, DualSPHysics v5.0 paper) on one B200.
  *
  * Reference for every call: /root/reference/PAPER.md (cited as PAPER.md:<line>) and the readings
- * A1..A20 / canonical definitions C1..C3 listed in DESIGN.md.
+ * A1..A23 / canonical definitions C1..C3 listed in DESIGN.md.
  *
  * General conventions
  *   - Every function returns SPH_OK (0) or a negative SPH_E_* code; nothing throws or exits.
@@ -147,13 +147,17 @@ int sph_set_motion(sph_ctx* ctx, int32_t group, int32_t axis, double stroke, dou
                    double phase);
 
 /* One neighbour-list build (cell key, radix sort, cell-range table, reorder) plus one
- * particle-interaction pass (Eq. 15, 17-18, 21-22, 28, 36) on the current state.
+ * particle-interaction pass (Eq. 15, 17-18 or 19-20, 21-22 or 23, 28, 36) on the current state.
  * Results: SPH_ACC, SPH_DRHODT, SPH_NBCOUNT and the dt candidates of Eq. 35. */
 int sph_compute_interactions(sph_ctx* ctx);
 
-/* nsteps symplectic predictor-corrector steps (Eq. 33-34) with the variable dt of
- * Eq. 35 taken from the pass at state n (A8).  Each step = 2 x (neighbour-list build + interaction
- * pass) + dt reduction + predictor + corrector, all on the device, no host synchronisation. */
+/* nsteps time steps with the variable dt of Eq. 35 taken from the pass at state n (A8), all on the device,
+ * no host synchronisation.
+ *   integrator 0: symplectic predictor-corrector (Eq. 33-34); each step = 2 x (neighbour-list
+ *                 build + interaction pass) + dt reduction + predictor + corrector.
+ *   integrator 1: Verlet (Eq. 30-31; A21); each step = neighbour-list build + interaction
+ *                 pass + dt reduction + update; step k since the last sph_load_particles uses Eq. 31 when
+ *                 k mod verlet_steps == 0, else Eq. 30. */
 int sph_step(sph_ctx* ctx, int32_t nsteps);
 
 /* Copy one field to host memory `dst` of `dst_bytes` bytes (must be at least the field's size, else
