@@ -256,10 +256,13 @@ def run_ours(args):
     achieved = per_pass * flops_per_inter / (pi_ms * 1e-3) / 1e12
     peak = fp32_peak_tflops(sm_max)
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "pi_dram_bytes_per_launch.json")
+    tpath = os.path.join(ROOT, "profiles", "pi_dram_bytes_per_launch.csv")   # from the ncu --set full captures
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"pi_kernel_{info0.pi_kernel}")
+            for row in open(tpath).read().splitlines()[1:]:
+                f = row.split(",")
+                if int(f[0]) == int(info0.pi_kernel):
+                    traffic = int(f[1])
         except Exception:
             traffic = None
     phases = {k: getattr(tm1, k) / args.steps for k in ("ms_key", "ms_sort", "ms_cellstart", "ms_reorder",
