@@ -17,6 +17,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # No -use_fast_math: the canonical predicate (C2) and conversions (C1) need IEEE mul/fma/div.
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC,-fvisibility=hidden", "-Xptxas", "-v"]
+FLAGS += os.environ.get("SPH_NVCC_EXTRA", "").split()      # e.g. -DQ_STATS (development counters; never in a release build)
 
 
 def _deps():

@@ -11,12 +11,14 @@
 //             half-precision test records of candidates 16g+r and 16g+r+8 (packed as half2), three HFMA2 and
 //             one HSET2 per a evaluate the expanded-form prefilter |b|^2 - 2 a.b < R^2 + margin - |a|^2 for
 //             both candidates at once.  The prefilter is conservative (margin > its rounding error, DESIGN.md
-//             5.2); the bits of both a are OR-ed into one 32-bit word per 16 steps; non-empty words go to a pool
-//             per quarter-warp in shared memory.
-//   P phase : (pair) the lanes of a quarter-warp claim the pool words dynamically, in (word, residue) order, so
-//             the 8 records loaded by a quarter-warp in one step lie in 8 different bank groups (two conflict-free
-//             LDS.128 per popped b) while the work stays balanced.  Every popped b is evaluated against BOTH a of
-//             the lane with packed FP32x2 arithmetic, b entering as a broadcast scalar operand.  The exact
+//             5.2); the bits of both a are OR-ed into one 32-bit word per 16 steps; non-empty words go to the
+//             lane's private word list in shared memory (no votes, no compaction across lanes).
+//   P phase : (pair) every lane pops the set bits of its own words (one FLO per pop).  Lane r only ever holds
+//             candidates of residue r, so the 8 records loaded by a quarter-warp in one step lie in 8 different
+//             bank groups (two conflict-free LDS.128 per popped b).  The trip count is the warp maximum of the
+//             per-lane pop counts (one REDUX per round), so the loop carries no vote.  Every popped b is
+//             evaluated against BOTH a of the lane with packed FP32x2 arithmetic, b entering as a broadcast
+//             scalar operand.  The exact
 //             canonical predicate C2 (fp32, individually rounded) decides membership; a b that is a neighbour
 //             of only one of the two a contributes exactly 0 to the other (the kernel weight is clamped at 0).
 //   reduce  : the partial sums of the 8 lanes of a quarter-warp are combined with 3 butterfly shuffles
@@ -25,6 +27,7 @@
 // What is kept from the paper: cell-linked list, particles sorted by cell, fp32 cell-relative positions
 // (PAPER.md:558, 572).  What differs: the thread-per-particle loop with a branch per candidate.
 #include <cuda_fp16.h>
+#include <stdio.h>
 
 #include "pi_common.cuh"
 
@@ -35,13 +38,19 @@ constexpr int QS = QT + 2;                // staged cells per axis
 constexpr int QNCELL = QS * QS * QS;      // 64 staged cells per type block
 constexpr int QNR = 2 * QNCELL;           // staged ranges: block 0 = boundary, block 1 = fluid
 constexpr int QNSEG = 2 * QT * QT * QT;   // a-segments: (block, centre cell)
-constexpr int QCAP = 64;                  // pool entries (non-empty words) per quarter-warp per round
+constexpr int QSLOT = 8;                  // non-empty words (32 candidates of the lane's residue each) per lane per round
 constexpr int QB = 4;                     // T-phase steps whose loads are issued together
 constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
 constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
 
 // offset of the staged range of row k = (dz + 1) * 3 + (dy + 1) relative to the row dy = dz = 0
 __constant__ int c_rowoff[9] = {-QS * QS - QS, -QS * QS, -QS * QS + QS, -QS, 0, QS, QS * QS - QS, QS * QS, QS * QS + QS};
+
+// A group of 16 a is processed as two work units (part 0, part 1) that cover disjoint rows of the stencil and add
+// their partial sums to the zeroed output with atomics: units of half the size halve the idle tail of a tile and
+// let the word lists of a unit fit one round.  part 0 = boundary-block rows + the centre and corner rows of the
+// fluid block, part 1 = the four edge rows of the fluid block (roughly equal numbers of neighbours).
+__constant__ int c_partrow[2][5] = {{4, 0, 2, 6, 8}, {1, 3, 5, 7, 7}};
 
 __device__ __forceinline__ int qrange(int blk, int ix, int iy, int iz) {   // staged indices, 0-based
   return ((blk * QS + iz) * QS + iy) * QS + ix;
@@ -50,8 +59,8 @@ __device__ __forceinline__ int qrange(int blk, int ix, int iy, int iz) {   // st
 struct QSmem {
   float4* rpos;       // (x, y, z, rho): exact tile-centred coordinates + density
   float4* rvel;       // (vx, vy, vz, P / rho)
-  uint4* tst;         // half2-packed test records: entry g*8 + r = candidates 16g+r (low halves) and 16g+r+8
-  uint2* bm;          // [warp][4][QCAP] pools: (bitmap word, byte address of the record of its bit 0)
+  uint2* tst;         // half-precision test record of every staged particle: (x, y), (z, |b|^2)
+  uint2* bm;          // [warp][QSLOT][32] private word lists: (bitmap word, byte address of the record of its bit 0)
   uint32_t* soff;     // QNR + 1
   uint32_t* gstart;   // QNR
   uint32_t* seg;      // [0] group counter, [1..QNSEG+1] a-group prefix
@@ -121,93 +130,124 @@ struct PairA {
   f2 x, y, z, vx, vy, vz, rho, inv_rho, kap;   // kap = P / rho
 };
 struct PairAcc2 {
-  f2 sx, sy, sz, sc, sd;
+  // raw sums of the two a of a lane, kept as scalars: plain FFMA accumulate in place, whereas ptxas copies a
+  // loop-carried FFMA2 destination back with two moves per sum (measured on the SASS of this kernel)
+  float sx[2], sy[2], sz[2], sc[2], sd[2];
   float visc0, visc1;
-  f2 nb;              // neighbour counts, kept as floats (exact integers)
+  float nb[2];        // neighbour counts, kept as floats (exact integers)
   f2 lx, ly, lz;      // laminar viscosity sums, Eq. 23 (LAM instantiations only)
 };
+// acc[h] += a_h * b_h
+__device__ __forceinline__ void f2_fma_acc2(f2 a, f2 b, float (&acc)[2]) {
+  acc[0] = fmaf(f2_lo(a), f2_lo(b), acc[0]);
+  acc[1] = fmaf(f2_hi(a), f2_hi(b), acc[1]);
+}
 
-// One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free.  A b outside the
-// support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record) gets weight 0:
-// w = max(1 - q/2, 0).  nb counts the exact canonical predicate C2.  pb = (x, y, z, rho_b), vb = (v_b, P_b/rho_b).
+// One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free, in two parts so that
+// the record registers are free again after the head (the P loop reloads them for the next step before the tail).
+// A b outside the support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record)
+// gets weight 0: w = max(1 - q/2, 0), and is masked out of the viscous dt candidate (A12) by the exact predicate.
+// nb counts the exact canonical predicate C2.  pb = (x, y, z, rho_b), vb = (v_b, P_b/rho_b).
 // DDT: this b enters the density diffusion term (A4).
+struct PairTmp {
+  f2 dux, duy, duz, dvx, dvy, dvz, drho, rs, ppb;
+  float inv_rho_b;
+};
+template <bool A_FLUID, bool DDT>
+__device__ __forceinline__ void pair2_head(const PairA& a, const float4 pb, const float4 vb, PairTmp& T) {
+  T.dux = f2_add(a.x, f2_bc(-pb.x));   // exact (C1)
+  T.duy = f2_add(a.y, f2_bc(-pb.y));
+  T.duz = f2_add(a.z, f2_bc(-pb.z));
+  T.dvx = f2_add(a.vx, f2_bc(-vb.x));
+  T.dvy = f2_add(a.vy, f2_bc(-vb.y));
+  T.dvz = f2_add(a.vz, f2_bc(-vb.z));
+  T.inv_rho_b = fast_rcp(pb.w);
+  if (A_FLUID) {
+    if (DDT) T.drho = f2_add(a.rho, f2_bc(-pb.w));
+    T.rs = f2_add(a.rho, f2_bc(pb.w));
+    T.ppb = f2_mul(a.inv_rho, f2_bc(vb.w));       // kap_b / rho_a
+  }
+}
 template <bool A_FLUID, bool DDT, bool LAM, bool FOURT>
-__device__ __forceinline__ void pair2(const DevConsts& C, const PairA& a, const float4 pb, const float4 vb,
-                                      PairAcc2& A) {
-  const f2 dux = f2_add(a.x, f2_bc(-pb.x));   // exact (C1)
-  const f2 duy = f2_add(a.y, f2_bc(-pb.y));
-  const f2 duz = f2_add(a.z, f2_bc(-pb.z));
-  f2 r2 = f2_mul(dux, dux);                   // C2: individually rounded
-  r2 = f2_fma(duy, duy, r2);
-  r2 = f2_fma(duz, duz, r2);
+__device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, const PairTmp& T, PairAcc2& A) {
+  f2 r2 = f2_mul(T.dux, T.dux);                   // C2: individually rounded
+  r2 = f2_fma(T.duy, T.duy, r2);
+  r2 = f2_fma(T.duz, T.duz, r2);
   const float r2a = f2_lo(r2), r2b = f2_hi(r2);
-  f2_add_acc(f2_pack(f_lt(r2a, C.R2u), f_lt(r2b, C.R2u)), A.nb);   // exact: counts stay far below 2^24
+  const f2 inside = f2_pack(f_lt(r2a, C.R2u), f_lt(r2b, C.R2u));
+  A.nb[0] += f2_lo(inside);                       // exact: counts stay far below 2^24
+  A.nb[1] += f2_hi(inside);
   f2 w = f2_fma(f2_pack(fast_sqrt(r2a), fast_sqrt(r2b)), f2_bc(-C.qscale), f2_bc(1.0f));   // 1 - q/2   (Eq. 11)
   w = f2_pack(fmaxf(f2_lo(w), 0.f), fmaxf(f2_hi(w), 0.f));
-  const f2 w3 = f2_mul(f2_mul(w, w), w);      // grad_a W_ab = Cf w^3 cs du
-  const float inv_rho_b = fast_rcp(pb.w);
-  const f2 dvx = f2_add(a.vx, f2_bc(-vb.x));
-  const f2 dvy = f2_add(a.vy, f2_bc(-vb.y));
-  const f2 dvz = f2_add(a.vz, f2_bc(-vb.z));
-  f2 dot = f2_mul(dvx, dux);                  // v_ab . r_ab / cs
-  dot = f2_fma(dvy, duy, dot);
-  dot = f2_fma(dvz, duz, dot);
-  const f2 gb = f2_mul(w3, f2_bc(inv_rho_b));
-  f2_fma_acc(gb, dot, A.sc);
+  const f2 w3 = f2_mul(f2_mul(w, w), w);          // grad_a W_ab = Cf w^3 cs du
+  f2 dot = f2_mul(T.dvx, T.dux);                  // v_ab . r_ab / cs
+  dot = f2_fma(T.dvy, T.duy, dot);
+  dot = f2_fma(T.dvz, T.duz, dot);
+  const f2 gb = f2_mul(w3, f2_bc(T.inv_rho_b));
+  f2_fma_acc2(gb, dot, A.sc);
   if (A_FLUID) {
     if (DDT) {
-      f2 drho = f2_add(a.rho, f2_bc(-pb.w));
+      f2 drho = T.drho;
       if (FOURT) {   // Eq. 19-20 (A23): minus rho^H_ab = e (k0 + e (k1 + e (k2 + e k3))), e = c_hyd . du
-        f2 e = f2_mul(dux, f2_bc(C.c_hyd[0]));
-        e = f2_fma(duy, f2_bc(C.c_hyd[1]), e);
-        e = f2_fma(duz, f2_bc(C.c_hyd[2]), e);
+        f2 e = f2_mul(T.dux, f2_bc(C.c_hyd[0]));
+        e = f2_fma(T.duy, f2_bc(C.c_hyd[1]), e);
+        e = f2_fma(T.duz, f2_bc(C.c_hyd[2]), e);
         f2 h = f2_fma(e, f2_bc(C.hyd_k[3]), f2_bc(C.hyd_k[2]));
         h = f2_fma(e, h, f2_bc(C.hyd_k[1]));
         h = f2_fma(e, h, f2_bc(C.hyd_k[0]));
         drho = f2_fma(f2_mul(e, f2_bc(-1.0f)), h, drho);
       }
-      f2_fma_acc(gb, drho, A.sd);
+      f2_fma_acc2(gb, drho, A.sd);
     }
-    const f2 rs = f2_add(a.rho, f2_bc(pb.w));
-    const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), rs);
+    const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), T.rs);
     const f2 xinv = f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den)));
     const f2 y = f2_mul(dot, xinv);                       // dot / ((r2 + eta2) rs)
     if (LAM) {                                            // Eq. 23: sum w^3 r2u / ((r2u + eta2u) rs) dv
       const f2 lam = f2_mul(f2_mul(w3, r2), xinv);
-      f2_fma_acc(lam, dvx, A.lx);
-      f2_fma_acc(lam, dvy, A.ly);
-      f2_fma_acc(lam, dvz, A.lz);
+      f2_fma_acc(lam, T.dvx, A.lx);
+      f2_fma_acc(lam, T.dvy, A.ly);
+      f2_fma_acc(lam, T.dvz, A.lz);
     }
-    const f2 mu = f2_mul(y, rs);                          // mu_ab / c_mu   (Eq. 21, A12)
+    const f2 mu = f2_mul(f2_mul(y, T.rs), inside);        // mu_ab / c_mu over accepted pairs only (Eq. 21, A12)
     A.visc0 = fmaxf(A.visc0, fabsf(f2_lo(mu)));
     A.visc1 = fmaxf(A.visc1, fabsf(f2_hi(mu)));
     const f2 t = f2_pack(fminf(f2_lo(y), 0.f), fminf(f2_hi(y), 0.f));   // approaching pairs only (Eq. 21)
     // (Pa + Pb) / (rho_a rho_b) = kap_a / rho_b + kap_b / rho_a
-    const f2 pp = f2_fma(a.kap, f2_bc(inv_rho_b), f2_mul(a.inv_rho, f2_bc(vb.w)));
+    const f2 pp = f2_fma(a.kap, f2_bc(T.inv_rho_b), T.ppb);
     const f2 coef = f2_mul(w3, f2_fma(f2_bc(C.c_pi), t, pp));
-    f2_fma_acc(coef, dux, A.sx);
-    f2_fma_acc(coef, duy, A.sy);
-    f2_fma_acc(coef, duz, A.sz);
+    f2_fma_acc2(coef, T.dux, A.sx);
+    f2_fma_acc2(coef, T.duy, A.sy);
+    f2_fma_acc2(coef, T.duz, A.sz);
   }
 }
 
-// Predicated 64-bit shared-memory load into an existing register pair (nothing happens if !p).
-__device__ __forceinline__ void lds64_if(bool p, unsigned saddr, unsigned& x, unsigned& y) {
-  asm volatile("{.reg .pred q; setp.ne.u32 q, %2, 0; @q ld.shared.v2.u32 {%0, %1}, [%3];}"
-               : "+r"(x), "+r"(y) : "r"((unsigned)p), "r"(saddr));
+__device__ __forceinline__ unsigned bfind32(unsigned x) {   // index of the highest set bit; 0xffffffff if x == 0
+  unsigned r;
+  asm("bfind.u32 %0, %1;" : "=r"(r) : "r"(x));
+  return r;
 }
 
-// Sum over the 8 lanes of a quarter-warp (butterfly, fixed order).
+// Take the next (word, base) entry of a lane's list if the current word is used up and the list is not:
+// one predicate drives the 64-bit shared-memory load and the pointer increment (nothing happens otherwise).
+__device__ __forceinline__ void next_word_if_empty(unsigned& cur, unsigned& base, unsigned& wptr, unsigned wend) {
+  asm volatile(
+      "{.reg .pred q;\n\t"
+      "setp.lt.u32 q, %2, %3;\n\t"
+      "setp.eq.and.u32 q, %0, 0, q;\n\t"
+      "@q ld.shared.v2.u32 {%0, %1}, [%2];\n\t"
+      "@q add.u32 %2, %2, 256;}"
+      : "+r"(cur), "+r"(base), "+r"(wptr) : "r"(wend));
+}
+
+// Sum over the 4 lanes that share a pair of a (butterfly, fixed order).
 __device__ __forceinline__ float qsum(float v) {
   v += __shfl_xor_sync(0xffffffffu, v, 1);
   v += __shfl_xor_sync(0xffffffffu, v, 2);
-  v += __shfl_xor_sync(0xffffffffu, v, 4);
   return v;
 }
 __device__ __forceinline__ float qmax(float v) {
   v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
   v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
-  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 4));
   return v;
 }
 __device__ __forceinline__ unsigned qsumu(unsigned v) {
@@ -217,20 +257,63 @@ __device__ __forceinline__ unsigned qsumu(unsigned v) {
   return v;
 }
 
-// One a-group: up to 8 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
-// A_FLUID ? 1 : 0, staged at [cell_start + 8*grp, ...).  bmw is this warp's pool area ([4][QCAP] uint2).
+#ifdef Q_STATS
+__device__ unsigned long long g_qstats[8];
+__global__ void k_qstats_print() {
+  printf("QSTATS warp_steps %llu pops %llu rounds %llu slots %llu groups %llu eff %.4f\n", g_qstats[0], g_qstats[1], g_qstats[2],
+         g_qstats[3], g_qstats[4], (double)g_qstats[1] / (32.0 * (double)g_qstats[0]));
+  for (int i = 0; i < 8; i++) g_qstats[i] = 0;
+}
+#endif
+
+// ---- TMA bulk copy global -> shared memory, completion counted in bytes on an mbarrier ----
+__device__ __forceinline__ void mbar_init(unsigned mbar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned mbar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned mbar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(mbar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, unsigned mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(mbar)
+               : "memory");
+}
+
+// m16n8k8 half-precision MMA with half accumulators: D (16 x 8) = A (16 x 8, row) * B (8 x 8, col) + C.
+// Lane (g = lane / 4, t = lane % 4) holds A[g][2t, 2t+1] and A[g+8][2t, 2t+1], B[2t, 2t+1][g], and the
+// same elements of C / D as of A.
+__device__ __forceinline__ void mma_m16n8k8(unsigned& d0, unsigned& d1, unsigned a0, unsigned a1, unsigned b0, unsigned c0,
+                                            unsigned c1) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f16.f16.f16.f16 {%0, %1}, {%2, %3}, {%4}, {%5, %6};"
+               : "=r"(d0), "=r"(d1) : "r"(a0), "r"(a1), "r"(b0), "r"(c0), "r"(c1));
+}
+
+// One a-group: up to 16 particles a of the centre cell (cx, cy, cz) (tile-local, 0..QT-1), type block
+// A_FLUID ? 1 : 0, staged at [cell_start + 16*grp, ...).  bmw is this warp's word-list area ([QSLOT][32] uint2).
+// Lane (g, t) = (lane / 4, lane % 4): the 4 lanes of g own the pair (a_2g, a_2g+1); lane t owns the candidates
+// whose staged index is congruent to 2t or 2t+1 modulo 8.
 template <bool A_FLUID, bool LAM, bool FOURT>
 __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint2* bmw, int cx,
-                                              int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp,
-                                              unsigned total, float& f2max, float& viscmax, unsigned int& nbsum) {
-  const int lane = threadIdx.x & 31, q = lane >> 3, r = lane & 7;
-  const unsigned t0 = grp * 8 + 2 * q, t1 = t0 + 1;
+                                              int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp, int part,
+                                              unsigned total, float& viscmax, unsigned int& nbsum) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  const unsigned t0 = grp * 16 + 2 * g, t1 = t0 + 1;
   const bool act0 = t0 < n_a, act1 = t1 < n_a;
   const unsigned ja0 = cell_start + (act0 ? t0 : 0), ja1 = cell_start + (act1 ? t1 : 0);
 
   // ---- state of the two a of this lane (inactive: far away, never accepted) ----
   PairA a;
-  __half2 nx0, ny0, nz0, th0, nx1, ny1, nz1, th1;
+  unsigned fa0, fa1, fc0, fc1;    // MMA fragments of the prefilter: rows g (a_2g) and g + 8 (a_2g+1)
   float rho_a0, rho_a1;
   {
     float4 p0 = S.rpos[ja0], v0 = S.rvel[ja0], p1 = S.rpos[ja1], v1 = S.rvel[ja1];
@@ -242,153 +325,191 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     a.inv_rho = f2_pack_pinned(fast_rcp(p0.w), fast_rcp(p1.w));
     a.vx = f2_pack_pinned(v0.x, v1.x); a.vy = f2_pack_pinned(v0.y, v1.y); a.vz = f2_pack_pinned(v0.z, v1.z);
     a.kap = f2_pack_pinned(v0.w, v1.w);
-    // prefilter operands (half precision): s = |b|^2 - 2 a.b  <  thr = R2u + margin - |a|^2
-    const float thr0 = act0 ? (C.R2u + Q_MARGIN) - fmaf(p0.z, p0.z, fmaf(p0.y, p0.y, p0.x * p0.x)) : -60000.f;
-    const float thr1 = act1 ? (C.R2u + Q_MARGIN) - fmaf(p1.z, p1.z, fmaf(p1.y, p1.y, p1.x * p1.x)) : -60000.f;
-    nx0 = __float2half2_rn(act0 ? -2.f * p0.x : 0.f); ny0 = __float2half2_rn(act0 ? -2.f * p0.y : 0.f);
-    nz0 = __float2half2_rn(act0 ? -2.f * p0.z : 0.f); th0 = __half2half2(__float2half_ru(thr0));
-    nx1 = __float2half2_rn(act1 ? -2.f * p1.x : 0.f); ny1 = __float2half2_rn(act1 ? -2.f * p1.y : 0.f);
-    nz1 = __float2half2_rn(act1 ? -2.f * p1.z : 0.f); th1 = __half2half2(__float2half_ru(thr1));
+    // Prefilter as a 16 x 8 x 8 product: row of a = (-2a_hi, 1, -2a_lo, 0) with -2a = hi + lo in
+    // half precision, column of b = (b, |b|^2, b, |b|^2), C = |a|^2 - R2u - margin, so that
+    // D = |b|^2 - 2 a.b + |a|^2 - (R2u + margin) and b is a candidate of a iff D < 0.  An inactive a has a zero
+    // row and C = +60000: never accepted.
+    float e0[3] = {-2.f * p0.x, -2.f * p0.y, -2.f * p0.z}, e1[3] = {-2.f * p1.x, -2.f * p1.y, -2.f * p1.z};
+    float k0a, k0b, k1a, k1b;       // elements (2t, 2t+1) of the two rows
+    {
+      float h0[3], l0[3], h1[3], l1[3];
+#pragma unroll
+      for (int k = 0; k < 3; k++) {
+        h0[k] = __half2float(__float2half_rn(e0[k])); l0[k] = e0[k] - h0[k];
+        h1[k] = __half2float(__float2half_rn(e1[k])); l1[k] = e1[k] - h1[k];
+      }
+      k0a = t == 0 ? h0[0] : t == 1 ? h0[2] : t == 2 ? l0[0] : l0[2];
+      k0b = t == 0 ? h0[1] : t == 1 ? 1.f : t == 2 ? l0[1] : 0.f;
+      k1a = t == 0 ? h1[0] : t == 1 ? h1[2] : t == 2 ? l1[0] : l1[2];
+      k1b = t == 0 ? h1[1] : t == 1 ? 1.f : t == 2 ? l1[1] : 0.f;
+    }
+    const float c0f = fmaf(p0.z, p0.z, fmaf(p0.y, p0.y, p0.x * p0.x)) - (C.R2u + Q_MARGIN);
+    const float c1f = fmaf(p1.z, p1.z, fmaf(p1.y, p1.y, p1.x * p1.x)) - (C.R2u + Q_MARGIN);
+    fa0 = act0 ? h2_as_u32(__floats2half2_rn(k0a, k0b)) : 0u;
+    fa1 = act1 ? h2_as_u32(__floats2half2_rn(k1a, k1b)) : 0u;
+    fc0 = h2_as_u32(__half2half2(act0 ? __float2half_rd(c0f) : __float2half_rn(60000.f)));   // rounded down: conservative
+    fc1 = h2_as_u32(__half2half2(act1 ? __float2half_rd(c1f) : __float2half_rn(60000.f)));
   }
+#ifdef Q_STATS
+  if (lane == 0) atomicAdd(&g_qstats[4], 1ull);
+#endif
   PairAcc2 acc;
-  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = acc.nb = acc.lx = acc.ly = acc.lz = f2_pack(0.f, 0.f);
+  acc.lx = acc.ly = acc.lz = f2_pack(0.f, 0.f);
+#pragma unroll
+  for (int hh = 0; hh < 2; hh++) acc.sx[hh] = acc.sy[hh] = acc.sz[hh] = acc.sc[hh] = acc.sd[hh] = acc.nb[hh] = 0.f;
   acc.visc0 = acc.visc1 = 0.f;
 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
   // term only if ddt_over_boundary, A4), then the 9 fluid rows; boundary a sweeps the fluid rows only (Eq. 36).
-  const int nruns = A_FLUID ? 18 : 9;
-  int ri = (A_FLUID && S.soff[QNCELL] == 0u) ? 9 : 0;   // no boundary particle staged: skip their 9 rows
-  int gw = -1, g_first = 0, g_last = -1;
-  unsigned j0 = 0, j1 = 0;
+  // Runs of this unit: fluid a, part 0: the 9 boundary-block rows, then 5 fluid rows; otherwise fluid rows only.
+  const int nbr = (A_FLUID && part == 0) ? 9 : 0;       // boundary-block runs come first
+  const int nruns = nbr + (part == 0 ? 5 : 4);
+  int ri = (nbr && S.soff[QNCELL] == 0u) ? nbr : 0;     // no boundary particle staged: skip their 9 rows
+  int sw = -1, s_last = -1;                             // next block of 8 candidates of the open run, its last block
+  int j0 = 0, j1 = 0;
   const unsigned dummy_addr = total * 16u;
   const int row0 = qrange(1, cx, 1 + cy, 1 + cz);        // fluid-block range of the cell left of the centre cell
-  uint2* bmq = bmw + q * QCAP;                       // pool of this quarter-warp
-  const unsigned bmq_s = (unsigned)__cvta_generic_to_shared(bmq);
-  const unsigned qsel = 0x4440u | (unsigned)q;           // byte_perm selector: byte q of a ballot
-  const unsigned lt_mask = (1u << r) - 1u;               // lanes of the quarter-warp below this one
+  uint2* wl = bmw + lane;                                // private word list of this lane: entries wl[32 * k]
+  const unsigned wl_s = (unsigned)__cvta_generic_to_shared(wl);
+  const uint32_t* tst32 = reinterpret_cast<const uint32_t*>(S.tst) + 2 * g + (t & 1);   // B fragment of block 0
 
   while (ri < nruns) {
-    // ================= T phase: fill the pools (until one of them would overflow) =================
-    const int ri_end = (A_FLUID && ri < 9) ? 9 : nruns;
-    const bool ddt_round = !(A_FLUID && ri < 9 && !C.ddt_over_boundary);
-    int nw = 0;
-    unsigned npool = 0;
+    // ================= T phase: fill the private word lists (at most QSLOT non-empty words per lane and round) =================
+    const int ri_end = ri < nbr ? nbr : nruns;
+    const bool ddt_round = !(ri < nbr && !C.ddt_over_boundary);
+    int nslot = 0;
+    unsigned nw = 0, npop = 0;
     while (ri < ri_end) {
-      if (gw < 0) {   // open run ri
+      // a slot adds up to two words to a list: if one might not fit, run the P phase first (the round resumes here)
+      if (__any_sync(0xffffffffu, nw > (unsigned)(QSLOT - 2))) break;
+      if (sw < 0) {   // open run ri
         // row ri of the stencil: cells (cx-1 .. cx+1, cy+dy, cz+dz) of one type block are one contiguous range
-        const int row = ((A_FLUID && ri < 9) ? row0 - QNCELL : row0) + c_rowoff[(A_FLUID && ri >= 9) ? ri - 9 : ri];
-        j0 = S.soff[row];
-        j1 = S.soff[row + 3];
+        const int row = ri < nbr ? row0 - QNCELL + c_rowoff[ri] : row0 + c_rowoff[c_partrow[part][ri - nbr]];
+        j0 = (int)S.soff[row];
+        j1 = (int)S.soff[row + 3];
         if (j1 <= j0) { ri++; continue; }
-        g_first = (int)(j0 >> 4);
-        g_last = (int)((j1 - 1) >> 4);
-        gw = g_first;
+        sw = j0 >> 3;
+        s_last = (j1 - 1) >> 3;
       }
-      const int nstep = min(16, g_last - gw + 1);
-      const uint4* tp = S.tst + gw * 8 + r;
-      unsigned u = 0;
-      // 16 steps in batches of QB: the loads of a batch are issued together, so that they overlap the
-      // arithmetic of the previous batch.  Steps beyond nstep read whatever follows (the test records are
-      // followed by the pools in shared memory, so the addresses stay valid); their bits are masked below.
+      // One slot = up to 32 steps; a step tests the 8 candidates of block sw + i against the 16 a of the warp with
+      // one MMA.  d0 | d1 carries the sign of D for (either a of the lane, candidate 8 (sw + i) + 2t) in bit 15 and
+      // for candidate + 1 in bit 31; two funnel shifts append them to the words of the two residue streams, so
+      // that after ne steps bit p of a word belongs to step ne - 1 - p.  The loads of QB steps are issued
+      // together.  Steps beyond the run read whatever follows (the test records are followed by the word lists
+      // in shared memory, so the addresses stay valid); their bits are masked below.
+      const int nstep = min(32, s_last - sw + 1);
+      const int ne = (nstep + QB - 1) & ~(QB - 1);       // steps executed
+      const uint32_t* tq = tst32 + sw * 16;
+      unsigned accL = 0, accH = 0;
 #pragma unroll
-      for (int b0 = 0; b0 < 16; b0 += QB) {
+      for (int b0 = 0; b0 < 32; b0 += QB) {
         if (b0 < nstep) {
-          uint4 t[QB];
+          unsigned bb[QB];
 #pragma unroll
-          for (int i = 0; i < QB; i++) t[i] = tp[(b0 + i) * 8];   // may run past the run (never past the pools)
+          for (int i = 0; i < QB; i++) bb[i] = tq[(b0 + i) * 16];   // may run past the run (never past the lists)
 #pragma unroll
           for (int i = 0; i < QB; i++) {
-            const __half2 bx = u32_as_h2(t[i].x), by = u32_as_h2(t[i].y), bz = u32_as_h2(t[i].z), bw = u32_as_h2(t[i].w);
-            const __half2 s0 = __hfma2(nz0, bz, __hfma2(ny0, by, __hfma2(nx0, bx, bw)));
-            const __half2 s1 = __hfma2(nz1, bz, __hfma2(ny1, by, __hfma2(nx1, bx, bw)));
-            const unsigned m = __hlt2_mask(s0, th0) | __hlt2_mask(s1, th1);
-            u |= m & (0x00010001u << (b0 + i));
+            unsigned d0, d1;
+            mma_m16n8k8(d0, d1, fa0, fa1, bb[i], fc0, fc1);
+            const unsigned x = d0 | d1;
+            accH = __funnelshift_l(x, accH, 1);
+            accL = __funnelshift_l(x << 16, accL, 1);
           }
         }
       }
-      // keep the candidates that lie inside the run [j0, j1): bit i (low half) is candidate c + 16 i, bit
-      // 16 + i is candidate c + 8 + 16 i with c = 16 gw + r.  Branch free; this also drops the steps >= nstep.
-      {
-        const int c = gw * 16 + r;
-        const int lo0 = max(((int)j0 - c + 15) >> 4, 0), lo1 = min(max(((int)j1 - c + 15) >> 4, 0), 16);
-        const int hi0 = max(((int)j0 - c + 7) >> 4, 0), hi1 = min(max(((int)j1 - c + 7) >> 4, 0), 16);
-        const unsigned mlo = (0xffffu >> (16 - lo1)) & (0xffffu << lo0);
-        const unsigned mhi = (0xffffu >> (16 - hi1)) & (0xffffu << hi0);
-        u &= (mlo & 0xffffu) | (mhi << 16);
+      // keep the candidates that lie inside the run [j0, j1): step i of stream h is candidate c0 + 8 i with
+      // c0 = 8 sw + 2t + h, valid for i in [ilo, ihi], i.e. bits ne - 1 - ihi .. ne - 1 - ilo.  Branch free.
+      const int cL = 8 * sw + 2 * t;
+#pragma unroll
+      for (int h = 0; h < 2; h++) {
+        const int c0 = cL + h;
+        const int ilo = max((j0 - c0 + 7) >> 3, 0), ihi = min((j1 - 1 - c0) >> 3, ne - 1);   // arithmetic shifts
+        const unsigned m = ihi >= ilo ? (0xffffffffu >> (31 - (ne - 1 - ilo))) & (0xffffffffu << (ne - 1 - ihi)) : 0u;
+        unsigned& w = h ? accH : accL;
+        w &= m;
+        // a non-empty word goes to this lane's list, together with the byte address of the record of its bit 0
+        // (bit p -> record address - 128 p); no other lane reads it
+        if (w != 0u) {
+          wl[nw * 32u] = make_uint2(w, (unsigned)(c0 + 8 * (ne - 1)) * 16u);
+          nw++;
+          npop += (unsigned)__popc(w);
+        }
       }
-      // non-empty words go to the pool of this quarter-warp, compacted in (word, residue) order, together
-      // with the byte address of the record of bit 0 (bit p -> + 256 (p & 15) + 128 (p >> 4))
-      {
-        const unsigned nzq = __byte_perm(__ballot_sync(0xffffffffu, u != 0u), 0u, qsel);
-        // a pool would overflow: run the P phase first; this word is recomputed in the next round (rare)
-        if (__any_sync(0xffffffffu, npool + (unsigned)__popc(nzq) > (unsigned)QCAP)) break;
-        if (u != 0u)
-          bmq[npool + (unsigned)__popc(nzq & lt_mask)] = make_uint2(u, ((unsigned)gw * 16u + (unsigned)r) * 16u);
-        npool += (unsigned)__popc(nzq);
-      }
-      nw++;
-      gw += 16;
-      if (gw > g_last) { ri++; gw = -1; }
+      nslot++;
+      sw += 32;
+      if (sw > s_last) { ri++; sw = -1; }
     }
-    if (nw == 0) continue;
-    __syncwarp();
+    if (nslot == 0) continue;
 
-    // ================= P phase: the 8 lanes of a quarter-warp claim words from their pool =================
-    // Words are claimed in pool order, so the 8 words in flight are (nearly always) 8 consecutive pool entries
-    // = 8 different residues: the record loads stay bank-conflict free while the work is balanced dynamically.
+    // ================= P phase: every lane pops the bits of its own words =================
+    // Lane t holds candidates of residues 2t and 2t + 1 only.  The trip count is the warp maximum of the pop
+    // counts; a lane that has run out of bits evaluates the dummy record (exactly zero contribution).
+    const unsigned nmax = __reduce_max_sync(0xffffffffu, npop);
+#ifdef Q_STATS
+    {
+      const unsigned tot = __reduce_add_sync(0xffffffffu, npop);
+      if (lane == 0) {
+        atomicAdd(&g_qstats[0], (unsigned long long)nmax);      // warp steps
+        atomicAdd(&g_qstats[1], (unsigned long long)tot);       // pops
+        atomicAdd(&g_qstats[2], 1ull);                          // rounds
+        atomicAdd(&g_qstats[3], (unsigned long long)nslot);     // word slots
+      }
+    }
+#endif
     const unsigned char* rp = reinterpret_cast<const unsigned char*>(S.rpos);
     const unsigned char* rv = reinterpret_cast<const unsigned char*>(S.rvel);
-    unsigned cur = 0, base = 0, next = 8;
-    if ((unsigned)r < npool) {
-      const uint2 e = bmq[r];
-      cur = e.x;
-      base = e.y;
-    }
-    // one step: claim (lanes whose word is used up take the next pool entries in lane order), pop the highest
-    // set bit and issue the loads of its record; then evaluate the record fetched by the previous step
-    // (software pipeline, two steps per loop trip so that records and accumulators ping-pong without moves).
-    // Pool words are non-empty, so "no word" means "pool used up"; a lane without work loads the dummy record.
-#define Q_FETCH(PB, VB)                                                                                \
+    unsigned cur = 0, base = 0;
+    unsigned wptr = wl_s;
+    const unsigned wend = wl_s + nw * 256u;
+    // one pop: take the next word if the current one is used up and turn its highest set bit into a record
+    // address.  Software pipeline, two steps per loop trip (records ping-pong without moves): while step k is
+    // evaluated, the record of step k + 1 is being loaded and the address of step k + 2 is popped; a lane out of
+    // bits gets the dummy record.
+#define Q_POP(ADDR)                                                                                    \
   {                                                                                                    \
-    const bool need = cur == 0u;                                                                       \
-    const unsigned nq = __byte_perm(__ballot_sync(0xffffffffu, need), 0u, qsel);                       \
-    const unsigned ei = next + (unsigned)__popc(nq & lt_mask);                                         \
-    next += (unsigned)__popc(nq);                                                                      \
-    lds64_if(need && ei < npool, bmq_s + ei * 8u, cur, base);                                          \
-    more = __any_sync(0xffffffffu, cur != 0u);                                                         \
-    const unsigned p = 31u - (unsigned)__clz((int)cur); /* cur == 0 -> p = 0xffffffff (unused) */      \
-    const unsigned addr = cur != 0u ? base + ((p & 15u) << 8) + ((p >> 4) << 7) : dummy_addr;          \
+    next_word_if_empty(cur, base, wptr, wend);                                                         \
+    const unsigned p = bfind32(cur); /* cur == 0 -> 0xffffffff (unused) */                              \
+    ADDR = cur != 0u ? base - (p << 7) : dummy_addr;                                                   \
     cur &= ~(1u << (p & 31u));                                                                         \
-    PB = *reinterpret_cast<const float4*>(rp + addr);                                                  \
-    VB = *reinterpret_cast<const float4*>(rv + addr);                                                  \
   }
+#define Q_LOAD(ADDR, PB, VB)                                                                           \
+  PB = *reinterpret_cast<const float4*>(rp + ADDR);                                                    \
+  VB = *reinterpret_cast<const float4*>(rv + ADDR);
 #define Q_LOOP(DDT)                                                                                    \
   {                                                                                                    \
     float4 pbA, vbA, pbB, vbB;                                                                         \
-    bool more;                                                                                         \
-    Q_FETCH(pbA, vbA)                                                                                  \
-    while (more) { /* single exit: at most one surplus evaluation of dummy records per round */        \
-      Q_FETCH(pbB, vbB)                                                                                \
-      pair2<A_FLUID, DDT, LAM, FOURT>(C, a, pbA, vbA, acc);                                                        \
-      Q_FETCH(pbA, vbA)                                                                                \
-      pair2<A_FLUID, DDT, LAM, FOURT>(C, a, pbB, vbB, acc);                                                        \
+    PairTmp T;                                                                                         \
+    unsigned addr;                                                                                     \
+    Q_POP(addr)                                                                                        \
+    Q_LOAD(addr, pbA, vbA)                                                                             \
+    Q_POP(addr)                                                                                        \
+    _Pragma("unroll 1")                                                                                \
+    for (unsigned k = 0; k < nmax; k += 2) { /* at most one surplus evaluation of dummy records */     \
+      Q_LOAD(addr, pbB, vbB)   /* record of step k + 1: its address was popped during step k - 1 */    \
+      Q_POP(addr)              /* address of step k + 2 */                                             \
+      pair2_head<A_FLUID, DDT>(a, pbA, vbA, T);                                                        \
+      pair2_tail<A_FLUID, DDT, LAM, FOURT>(C, a, T, acc);                                              \
+      Q_LOAD(addr, pbA, vbA)                                                                           \
+      Q_POP(addr)                                                                                      \
+      pair2_head<A_FLUID, DDT>(a, pbB, vbB, T);                                                        \
+      pair2_tail<A_FLUID, DDT, LAM, FOURT>(C, a, T, acc);                                              \
     }                                                                                                  \
   }
     if (ddt_round) Q_LOOP(true) else Q_LOOP(false)
 #undef Q_LOOP
-#undef Q_FETCH
-    __syncwarp();
+#undef Q_LOAD
+#undef Q_POP
   }
 
-  // ---- combine the 8 lanes of each quarter-warp; lane r = 0 writes both particles ----
+  // ---- combine the 4 lanes of each pair; lane t = 0 writes both particles ----
   PairAcc r0 = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, r1 = r0;
-  r0.sc = qsum(f2_lo(acc.sc)); r1.sc = qsum(f2_hi(acc.sc));
-  const unsigned nb0 = (unsigned)qsum(f2_lo(acc.nb)), nb1 = (unsigned)qsum(f2_hi(acc.nb));
+  r0.sc = qsum(acc.sc[0]); r1.sc = qsum(acc.sc[1]);
+  const unsigned nb0 = (unsigned)qsum(acc.nb[0]), nb1 = (unsigned)qsum(acc.nb[1]);
   if (A_FLUID) {
-    r0.sx = qsum(f2_lo(acc.sx)); r1.sx = qsum(f2_hi(acc.sx));
-    r0.sy = qsum(f2_lo(acc.sy)); r1.sy = qsum(f2_hi(acc.sy));
-    r0.sz = qsum(f2_lo(acc.sz)); r1.sz = qsum(f2_hi(acc.sz));
-    r0.sd = qsum(f2_lo(acc.sd)); r1.sd = qsum(f2_hi(acc.sd));
+    r0.sx = qsum(acc.sx[0]); r1.sx = qsum(acc.sx[1]);
+    r0.sy = qsum(acc.sy[0]); r1.sy = qsum(acc.sy[1]);
+    r0.sz = qsum(acc.sz[0]); r1.sz = qsum(acc.sz[1]);
+    r0.sd = qsum(acc.sd[0]); r1.sd = qsum(acc.sd[1]);
     r0.visc = qmax(acc.visc0); r1.visc = qmax(acc.visc1);
     if (LAM) {
       r0.lx = qsum(f2_lo(acc.lx)); r1.lx = qsum(f2_hi(acc.lx));
@@ -396,7 +517,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       r0.lz = qsum(f2_lo(acc.lz)); r1.lz = qsum(f2_hi(acc.lz));
     }
   }
-  if (r == 0) {
+  if (t == 0) {
     const int ra = qrange(A_FLUID ? 1 : 0, 1 + cx, 1 + cy, 1 + cz);
     const unsigned gbase = S.gstart[ra] - S.soff[ra];
 #pragma unroll
@@ -404,17 +525,44 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       if (h == 0 ? act0 : act1) {
         const PairAcc& pa1 = h ? r1 : r0;
         unsigned nb = h ? nb1 : nb0;
-        if (A_FLUID) nb -= 1u;   // the particle itself passed the test at r = 0 and contributed exactly 0 (A17)
+        if (A_FLUID && part == 0) nb -= 1u;   // the particle itself (centre row) passed the test at r = 0, contributing exactly 0 (A17)
         const unsigned ga = gbase + (h ? ja1 : ja0);
-        const float4 out = finish_particle(C, A_FLUID, h ? rho_a1 : rho_a0, pa1);
-        A.acc[ga] = out;
-        if (A.nbcount) A.nbcount[ga] = nb;
-        if (A_FLUID) f2max = fmaxf(f2max, fmaf(out.x, out.x, fmaf(out.y, out.y, out.z * out.z)));
+        const float rho_a = h ? rho_a1 : rho_a0;
+        // scaled partial sums of this unit (finish_particle of pi_common.cuh, with g entering through part 0 only);
+        // the two units of a group add into the zeroed output: x1 + x2 is the same in either order
+        float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (A_FLUID) {
+          out.x = fmaf(C.c_mom, pa1.sx, part == 0 ? C.g[0] : 0.f);
+          out.y = fmaf(C.c_mom, pa1.sy, part == 0 ? C.g[1] : 0.f);
+          out.z = fmaf(C.c_mom, pa1.sz, part == 0 ? C.g[2] : 0.f);
+          if (LAM) {
+            out.x = fmaf(C.c_lam, pa1.lx, out.x);
+            out.y = fmaf(C.c_lam, pa1.ly, out.y);
+            out.z = fmaf(C.c_lam, pa1.lz, out.z);
+          }
+          out.w = fmaf(rho_a * C.c_cont, pa1.sc, C.c_ddt * pa1.sd);
+        } else {
+          out.w = rho_a * C.c_cont * pa1.sc;
+        }
+        atomicAdd(&A.acc[ga], out);
+        if (A.nbcount) atomicAdd(&A.nbcount[ga], nb);
         viscmax = fmaxf(viscmax, pa1.visc * C.c_mu);
         nbsum += nb;
       }
     }
   }
+}
+
+// max_a |F_a|^2 over the fluid particles (dt candidate of Eq. 35), from the summed output of the work units.
+__global__ void __launch_bounds__(256) k_quad_fmax(DevConsts C, const float4* __restrict__ acc,
+                                                   const uint32_t* __restrict__ cellstart, DevScalars* sc) {
+  const uint32_t f0 = cellstart[C.ncells], f1 = cellstart[2u * C.ncells];   // the fluid block in sorted order (C3)
+  float f2 = 0.f;
+  for (uint32_t i = f0 + blockIdx.x * blockDim.x + threadIdx.x; i < f1; i += gridDim.x * blockDim.x) {
+    const float4 o = acc[i];
+    f2 = fmaxf(f2, fmaf(o.x, o.x, fmaf(o.y, o.y, o.z * o.z)));
+  }
+  reduce_scalars(sc, f2, 0.f, 0u);
 }
 
 // Active-tile list: most tiles of a dam break are air.  A tile is active if its centre cells hold a particle;
@@ -445,17 +593,24 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   QSmem S;
   S.rpos = reinterpret_cast<float4*>(smem_raw);
   S.rvel = S.rpos + NMAX;
-  S.tst = reinterpret_cast<uint4*>(S.rvel + NMAX);
-  S.bm = reinterpret_cast<uint2*>(S.tst + (NMAX / 16) * 8);
-  S.soff = reinterpret_cast<uint32_t*>(S.bm + NWARP * 4 * QCAP);
+  S.tst = reinterpret_cast<uint2*>(S.rvel + NMAX);
+  S.bm = S.tst + NMAX;
+  S.soff = reinterpret_cast<uint32_t*>(S.bm + NWARP * QSLOT * 32);
   S.gstart = S.soff + (QNR + 1);
   S.seg = S.gstart + QNR;
   __shared__ uint32_t s_cnt[QNR];
   __shared__ uint32_t s_tile;
+  __shared__ __align__(8) unsigned long long s_mbar;
+  const unsigned mbar_s = (unsigned)__cvta_generic_to_shared(&s_mbar);
+  unsigned mbar_phase = 0;
+  if (threadIdx.x == 0) {
+    mbar_init(mbar_s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t n_active = A.tile_ws[0];
-  float f2max = 0.f, viscmax = 0.f;
+  float f2max = 0.f, viscmax = 0.f;   // f2max: overflow path only (k_quad_fmax covers every fluid particle)
   unsigned int nbsum = 0;
 
  for (;;) {
@@ -532,7 +687,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
       uint32_t n = 0;
       if (cx < vx && cy < vy && cz < vz && cz >= czlo && cz <= czhi) n = s_cnt[qrange(blk, 1 + cx, 1 + cy, 1 + cz)];
       S.seg[1 + s] = run;
-      run += (n + 7) / 8;
+      run += (n + 15) / 16;
     }
     S.seg[1 + QNSEG] = run;
     S.seg[0] = 0;
@@ -558,20 +713,42 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     continue;
   }
 
-  // 2. stage particles with tile-centred coordinates: u + integer cell offset - QT/2.  Exact: every value is a
-  //    multiple of 2^-22 with magnitude <= 2, so all differences are exact in fp32 (C1/C2).
+  // 2. stage the particles: the sorted arrays hold every cell as one contiguous range (C3), so each non-empty staged
+  //    range is two TMA bulk copies (positions + density, velocities + pressure) straight into shared memory,
+  //    completing on one mbarrier (no register staging, all copies of the tile in flight at once).
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic-proxy accesses of this memory come first
+  if (tid == 0) mbar_arrive_expect_tx(mbar_s, total * 32u);
+  for (int rr = tid; rr < QNR; rr += NT) {
+    const uint32_t n = s_cnt[rr];
+    if (n == 0) continue;
+    const uint32_t g0 = S.gstart[rr], d0 = S.soff[rr];
+    bulk_g2s(S.rpos + d0, A.posu + g0, n * 16u, mbar_s);
+    bulk_g2s(S.rvel + d0, A.velp + g0, n * 16u, mbar_s);
+  }
+  mbar_wait(mbar_s, mbar_phase);
+  mbar_phase ^= 1u;
+  // 3. in place: tile-centred coordinates u + integer cell offset - QT/2 (exact: every value is a multiple of
+  //    2^-22 with magnitude <= 2, so all differences are exact in fp32, C1/C2), P -> P / rho, and the
+  //    half-precision test records (x, y, z, |b|^2 of the rounded coordinates): the columns of the prefilter product
   for (int rr = warp; rr < QNR; rr += NWARP) {
     const uint32_t n = s_cnt[rr];
     if (n == 0) continue;
     const int c = rr % QNCELL;
     const float fx = (float)(c % QS - 1) - 0.5f * QT, fy = (float)((c / QS) % QS - 1) - 0.5f * QT,
                 fz = (float)(c / (QS * QS) - 1) - 0.5f * QT;
-    const uint32_t g0 = S.gstart[rr], d0 = S.soff[rr];
+    const uint32_t d0 = S.soff[rr];
     for (uint32_t i = lane; i < n; i += 32) {
-      const float4 p = A.posu[g0 + i];
-      const float4 v = A.velp[g0 + i];
-      S.rpos[d0 + i] = make_float4(p.x + fx, p.y + fy, p.z + fz, p.w);
-      S.rvel[d0 + i] = make_float4(v.x, v.y, v.z, __fdiv_rn(v.w, p.w));   // (v, P / rho)
+      float4 pp = S.rpos[d0 + i];
+      pp.x += fx; pp.y += fy; pp.z += fz;
+      S.rpos[d0 + i] = pp;
+      float* kap = reinterpret_cast<float*>(S.rvel + d0 + i) + 3;
+      *kap = __fdiv_rn(*kap, pp.w);                                       // (v, P / rho)
+      const __half2 hxy = __floats2half2_rn(pp.x, pp.y);
+      const __half hz = __float2half_rn(pp.z);
+      const float2 fxy = __half22float2(hxy);
+      const float gz = __half2float(hz);
+      const float w = fmaf(gz, gz, fmaf(fxy.y, fxy.y, fxy.x * fxy.x));
+      S.tst[d0 + i] = make_uint2(h2_as_u32(hxy), h2_as_u32(__halves2half2(hz, __float2half_rn(w))));
     }
   }
   if (tid == 0) {   // dummy record: popped by lanes that have run out of work, never within any support
@@ -579,41 +756,23 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     S.rvel[total] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
   __syncthreads();
-  // 3. half-precision test records, two candidates per half2: entry g*8 + r <- candidates 16g + r, 16g + r + 8
-  {
-    const uint32_t nent = ((total + 15) / 16) * 8;
-    for (uint32_t e = tid; e < nent; e += NT) {
-      const uint32_t c0 = (e >> 3) * 16 + (e & 7), c1 = c0 + 8;
-      float4 p0 = make_float4(0.f, 0.f, 0.f, 0.f), p1 = p0;
-      if (c0 < total) p0 = S.rpos[c0];
-      if (c1 < total) p1 = S.rpos[c1];
-      const __half2 hx = __floats2half2_rn(p0.x, p1.x), hy = __floats2half2_rn(p0.y, p1.y),
-                    hz = __floats2half2_rn(p0.z, p1.z);
-      const float2 fx = __half22float2(hx), fy = __half22float2(hy), fz = __half22float2(hz);
-      float w0 = fmaf(fz.x, fz.x, fmaf(fy.x, fy.x, fx.x * fx.x));   // |b|^2 of the rounded coordinates
-      float w1 = fmaf(fz.y, fz.y, fmaf(fy.y, fy.y, fx.y * fx.y));
-      if (c0 >= total) w0 = 60000.f;                                 // padding: never accepted
-      if (c1 >= total) w1 = 60000.f;
-      const __half2 hw = __floats2half2_rn(w0, w1);
-      S.tst[e] = make_uint4(h2_as_u32(hx), h2_as_u32(hy), h2_as_u32(hz), h2_as_u32(hw));
-    }
-  }
-  __syncthreads();
 
   // 4. a-groups, taken dynamically by the warps
-  uint2* bmw = S.bm + warp * 4 * QCAP;
+  uint2* bmw = S.bm + warp * QSLOT * 32;
   while (true) {
     uint32_t gi = 0;
     if (lane == 0) gi = atomicAdd(&S.seg[0], 1u);
     gi = __shfl_sync(0xffffffffu, gi, 0);
-    if (gi >= ngroups) break;
+    if (gi >= 2u * ngroups) break;
+    const int part = gi >= ngroups;                 // all units of part 0 (the larger ones) are handed out first
+    gi -= (uint32_t)part * ngroups;
     int s = 0;
     while (s + 1 < QNSEG && gi >= S.seg[1 + s + 1]) s++;
     const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
     const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
     const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
-    if (blk == 1) process_group<true, LAM, FOURT>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
-    else process_group<false, false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, total, f2max, viscmax, nbsum);
+    if (blk == 1) process_group<true, LAM, FOURT>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
+    else process_group<false, false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
   }
   if (part == 0) break;
   }   // parts
@@ -625,8 +784,8 @@ template <int NT, int NMAX, bool LAM, bool FOURT>
 int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
   constexpr int NWARP = NT / 32;
-  const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint4) * (NMAX / 16) * 8 +
-                      sizeof(uint2) * NWARP * 4 * QCAP + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
+  const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint2) * NMAX +
+                      sizeof(uint2) * NWARP * QSLOT * 32 + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM, FOURT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
@@ -649,8 +808,15 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
     }
   }
   if (cudaMemsetAsync(A.tile_ws, 0, 4 * sizeof(uint32_t), s) != cudaSuccess) return -1;
+  // the work units add their partial sums into the outputs
+  if (cudaMemsetAsync(A.acc, 0, sizeof(float4) * (size_t)A.n, s) != cudaSuccess) return -1;
+  if (A.nbcount && cudaMemsetAsync(A.nbcount, 0, sizeof(uint32_t) * (size_t)A.n, s) != cudaSuccess) return -1;
   k_quad_tiles<<<(unsigned)((ntiles + 255) / 256), 256, 0, s>>>(C, A.cellstart, ntx, nty, (int)ntiles, A.tile_ws);
   k_pi_quad<NT, NMAX, LAM, FOURT><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
+#ifdef Q_STATS
+  k_qstats_print<<<1, 1, 0, s>>>();
+#endif
+  k_quad_fmax<<<n_sm * 4, 256, 0, s>>>(C, A.acc, A.cellstart, A.sc);
   return 0;
 }
 
