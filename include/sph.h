@@ -15,8 +15,10 @@
  *     params.cuda_stream (a cudaStream_t; NULL = legacy default stream).
  *   - Calls are asynchronous on that stream except sph_load_particles (synchronous H2D from
  *     pageable memory), sph_read_state, sph_get_info and sph_get_timings, which synchronise it.
- *   - Asynchronous device-side faults (NaN in an acceleration, > 2^32-2 keys) set a device flag
- *     that the next synchronising call reports as SPH_E_NAN / SPH_E_OVERFLOW.
+ *   - Asynchronous device-side faults (a non-finite acceleration or density rate in an interaction
+ *     pass, a non-finite state in an update) set device flag bit 0, which the next sph_get_info
+ *     reports as SPH_E_NAN.  SPH_E_OVERFLOW is a host-side result only (grid too large for 32-bit
+ *     keys at sph_create, destination buffer too small at sph_read_state); flag bit 1 is reserved.
  *   - One context per host thread at a time.  There is no CPU fallback: without a CUDA device
  *     sph_create fails with SPH_E_CUDA.
  */
@@ -95,7 +97,7 @@ typedef struct sph_info {
   int64_t steps_done;
   double t, dt;            /* simulated time and last step's dt                                      */
   int32_t pi_kernel;       /* kernel actually used                                                   */
-  int32_t device_flags;    /* bit 0: non-finite value seen; bit 1: key overflow                      */
+  int32_t device_flags;    /* bit 0: non-finite value seen; bit 1: reserved                          */
 } sph_info;
 
 /* Accumulated device time per phase, measured with CUDA events on the context's stream while
@@ -172,7 +174,8 @@ int sph_get_info(sph_ctx* ctx, sph_info* info);
 int sph_set_profiling(sph_ctx* ctx, int32_t on);
 int sph_get_timings(sph_ctx* ctx, sph_timings* out);
 
-/* Message of the last error on this context ("" if none).  Valid until the next call. */
+/* Message of the last error on this context ("" if none).  Valid until the next call.
+ * With ctx = NULL: the reason of the last failed sph_create on the calling thread. */
 const char* sph_last_error(const sph_ctx* ctx);
 
 /* Library version string, e.g. "sph_b200 0.1 (sm_100a)". */

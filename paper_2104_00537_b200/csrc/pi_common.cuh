@@ -198,6 +198,7 @@ __device__ __forceinline__ void gather_one(const DevConsts& C, const PiArgs& A, 
     }
   }
   const float4 out = finish_particle(C, a_fluid, pa.w, S);
+  if (!isfinite(out.x + out.y + out.z + out.w)) atomicOr(&A.sc->flags, 1u);   // reported as SPH_E_NAN
   A.acc[a] = out;
   if (A.nbcount) A.nbcount[a] = nb;
   if (a_fluid) f2 = fmaxf(f2, fmaf(out.x, out.x, fmaf(out.y, out.y, out.z * out.z)));

@@ -544,6 +544,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
         } else {
           out.w = rho_a * C.c_cont * pa1.sc;
         }
+        if (!isfinite(out.x + out.y + out.z + out.w)) atomicOr(&A.sc->flags, 1u);   // reported as SPH_E_NAN
         atomicAdd(&A.acc[ga], out);
         if (A.nbcount) atomicAdd(&A.nbcount[ga], nb);
         viscmax = fmaxf(viscmax, pa1.visc * C.c_mu);
@@ -786,27 +787,16 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   constexpr int NWARP = NT / 32;
   const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint2) * NMAX +
                       sizeof(uint2) * NWARP * QSLOT * 32 + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM, FOURT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
-        cudaSuccess) {
-      cudaGetLastError();
-      return -1;
-    }
-    configured = true;
+  // per device, so set on every launch (a cheap host call): a process may hold contexts on several devices
+  if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM, FOURT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+      cudaSuccess) {
+    cudaGetLastError();
+    return -1;
   }
   const long long ntiles = (long long)ntx * nty * ntz;
   if (ntiles > 0x7fffffffLL || A.tile_ws == nullptr) return -1;
-  static int n_sm = 0;
-  if (n_sm == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) {
-      cudaGetLastError();
-      n_sm = 0;
-      return -1;
-    }
-  }
+  const int n_sm = A.n_sm;                            // of the context's device (sph_create)
+  if (n_sm <= 0) return -1;
   if (cudaMemsetAsync(A.tile_ws, 0, 4 * sizeof(uint32_t), s) != cudaSuccess) return -1;
   // the work units add their partial sums into the outputs
   if (cudaMemsetAsync(A.acc, 0, sizeof(float4) * (size_t)A.n, s) != cudaSuccess) return -1;

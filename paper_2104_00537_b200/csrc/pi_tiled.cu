@@ -242,6 +242,7 @@ __device__ __forceinline__ void process_chunk(const DevConsts& C, const PiArgs& 
     const int r_a = range_index<DIM>(blk_a, 1 + cxa, DIM == 3 ? 1 + cy : 0, 1 + cz);
     const unsigned ga = S.gstart[r_a] + (ja - S.soff[r_a]);
     const float4 out = finish_particle(C, A_FLUID, a.rho, acc);
+    if (!isfinite(out.x + out.y + out.z + out.w)) atomicOr(&A.sc->flags, 1u);   // reported as SPH_E_NAN
     A.acc[ga] = out;
     if (A.nbcount) A.nbcount[ga] = nb;
     if (A_FLUID) f2max = fmaxf(f2max, fmaf(out.x, out.x, fmaf(out.y, out.y, out.z * out.z)));
@@ -411,14 +412,11 @@ int launch_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntz = (C.nc[2] + T::TZ - 1) / T::TZ;
   const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint2) * PT_RQ * NT + sizeof(float) * NMAX +
                       sizeof(uint32_t) * (T::NR + 1 + T::NR + 2 + T::NSEG);
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(k_pi_tiled<DIM, NT, NMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
-        cudaSuccess) {
-      cudaGetLastError();
-      return -1;
-    }
-    configured = true;
+  // per device, so set on every launch (a cheap host call): a process may hold contexts on several devices
+  if (cudaFuncSetAttribute(k_pi_tiled<DIM, NT, NMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+      cudaSuccess) {
+    cudaGetLastError();
+    return -1;
   }
   const long long ntiles = (long long)ntx * nty * ntz;
   if (ntiles > 0x7fffffffLL) return -1;

@@ -29,6 +29,7 @@ struct sph_ctx {
 
   int64_t n = 0, cap = 0;
   bool loaded = false, nl_valid = false;
+  bool has_build = false, has_pass = false;   // since the last load: a neighbour-list build / an interaction pass
   ParticleSet set[2];
   int cur = 0;
   float4* acc = nullptr;
@@ -44,6 +45,7 @@ struct sph_ctx {
   std::vector<Motion> motions;
   Motion* d_motions = nullptr;
   int pi_kernel = 1;
+  int n_sm = 0;               // multiprocessors of the device this context was created on
   int integrator = 0, verlet_steps = 40;
   int64_t kstep = 0;          // Verlet step counter since the last load (Eq. 31 every verlet_steps)
 
@@ -62,6 +64,14 @@ int fail(sph_ctx* c, int code, const char* fmt, const char* detail = "") {
     snprintf(buf, sizeof(buf), fmt, detail);
     c->err = buf;
   }
+  return code;
+}
+
+// sph_create has no context to hang a message on: the reason of its last failure on this thread is kept here and
+// returned by sph_last_error(NULL).
+thread_local std::string g_create_err;
+int create_fail(int code, const std::string& why) {
+  g_create_err = why;
   return code;
 }
 
@@ -191,6 +201,10 @@ int derive(const sph_params* p, DevConsts& C, std::string& why) {
     if (nk > 2.0e9) { why = "grid too large"; return SPH_E_OVERFLOW; }
     C.nc[k] = (int)nk;
     ncells *= nk;
+    if (C.per[k] && fabs(ext - rint(ext)) > 1e-9 * ext) {
+      why = "periodic length must be an integer multiple of the cell size (pass cell_size = L / floor(L / (2h/cell_div)))";
+      return SPH_E_BADARG;
+    }
     if (C.per[k] && C.nc[k] < 2 * C.k + 1) { why = "periodic axis needs at least 2*cell_div+1 cells"; return SPH_E_BADARG; }
   }
   if (2.0 * ncells + 2.0 >= 4294967295.0 || ncells >= 2147483647.0) { why = "2*ncells+2 does not fit 32-bit keys"; return SPH_E_OVERFLOW; }
@@ -280,6 +294,7 @@ int build_nl(sph_ctx* ctx, bool with_n_state) {
   }
   ctx->n_nl += 1;
   ctx->nl_valid = true;
+  ctx->has_build = true;
   CK(cudaGetLastError());
   return SPH_OK;
 }
@@ -300,6 +315,7 @@ int run_pi(sph_ctx* ctx) {
   A.sc = ctx->sc;
   A.n = ctx->n;
   A.tile_ws = ctx->tile_ws;
+  A.n_sm = ctx->n_sm;
   bool done = false;
   if (ctx->pi_kernel == 3) {
     done = pi_quad(ctx->C, A, s) == 0;
@@ -310,8 +326,9 @@ int run_pi(sph_ctx* ctx) {
     pi_gather(ctx->C, A, s);
     if (ctx->pi_kernel == 2) ctx->pi_kernel = 1;   // configuration not supported by the tiled kernel
   }
-  ctx->n_launch += ctx->pi_kernel == 3 ? 3 : 2;   // reset + PI kernel (+ the quad kernel's active-tile list)
+  ctx->n_launch += ctx->pi_kernel == 3 ? 4 : 2;   // reset + PI kernel (+ the quad kernel's active-tile list and |F|max pass)
   ctx->n_pi += 1;
+  ctx->has_pass = true;
   CK(cudaGetLastError());
   return SPH_OK;
 }
@@ -326,25 +343,35 @@ int check_flags(sph_ctx* ctx, const DevScalars& h) {
 
 SPH_EXPORT const char* sph_version(void) { return "sph_b200 0.1 (sm_100a)"; }
 
-SPH_EXPORT const char* sph_last_error(const sph_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+SPH_EXPORT const char* sph_last_error(const sph_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
-  if (!params || !out) return SPH_E_BADARG;
+  if (!params || !out) return create_fail(SPH_E_BADARG, "null params or out pointer");
   *out = nullptr;
+  g_create_err.clear();
   std::string why;
   int rc = validate(params, why);
-  if (rc != SPH_OK) return rc;
+  if (rc != SPH_OK) return create_fail(rc, why);
   sph_ctx* ctx = new (std::nothrow) sph_ctx();
-  if (!ctx) return SPH_E_NOMEM;
+  if (!ctx) return create_fail(SPH_E_NOMEM, "out of host memory");
   ctx->prm = *params;
   rc = derive(params, ctx->C, why);
-  if (rc != SPH_OK) { delete ctx; return rc; }
+  if (rc != SPH_OK) { delete ctx; return create_fail(rc, why); }
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
   if (e != cudaSuccess || ndev == 0) {       // no CPU fallback: fail loudly
     cudaGetLastError();
     delete ctx;
-    return SPH_E_CUDA;
+    return create_fail(SPH_E_CUDA, "no usable CUDA device (there is no CPU fallback)");
+  }
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || ctx->n_sm <= 0) {
+      cudaGetLastError();
+      delete ctx;
+      return create_fail(SPH_E_CUDA, "cannot query the CUDA device");
+    }
   }
   ctx->stream = (cudaStream_t)params->cuda_stream;
   ctx->nkeys = 2u * ctx->C.ncells + 1u;      // keys 0 .. 2*ncells (C3)
@@ -361,12 +388,12 @@ SPH_EXPORT int sph_create(const sph_params* params, sph_ctx** out) {
   if (!ctx->cellstart || !ctx->sc || !ctx->digit_total || !ctx->tile_ws) {
     free_all(ctx);
     delete ctx;
-    return SPH_E_NOMEM;
+    return create_fail(SPH_E_NOMEM, "device allocation failed (cell table)");
   }
   if (cudaMemsetAsync(ctx->sc, 0, sizeof(DevScalars), ctx->stream) != cudaSuccess) {
     free_all(ctx);
     delete ctx;
-    return SPH_E_CUDA;
+    return create_fail(SPH_E_CUDA, "cudaMemsetAsync failed");
   }
   *out = ctx;
   return SPH_OK;
@@ -387,8 +414,17 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
   if (n < 0 || n > 0x7fffffff - 8192) return fail(ctx, SPH_E_BADARG, "n out of range");
   if (n > 0 && (!pos || !vel || !rho || !type)) return fail(ctx, SPH_E_BADARG, "null input array");
   cudaStream_t s = ctx->stream;
+  // a failed (re)load leaves the context unloaded, never half-valid
+  ctx->loaded = false;
+  ctx->has_build = ctx->has_pass = false;
+  ctx->nl_valid = false;
   if (n > ctx->cap || !ctx->acc) {            // (re)allocate particle storage
     cudaStreamSynchronize(s);
+    ctx->n = 0;
+    ctx->acc = nullptr;
+    ctx->nbcount = nullptr;
+    ctx->block_hist = nullptr;
+    for (int i = 0; i < 2; i++) { ctx->key[i] = ctx->idx[i] = nullptr; ctx->set[i] = ParticleSet(); }
     void* keep[] = {ctx->cellstart, ctx->sc, ctx->digit_total, ctx->tile_ws, ctx->d_motions};
     std::vector<void*> old = ctx->allocs;
     for (void* p : old) {
@@ -550,9 +586,10 @@ SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst
     default: return fail(ctx, SPH_E_BADARG, "unknown field");
   }
   if (dst_bytes < need) return fail(ctx, SPH_E_OVERFLOW, "destination buffer too small");
-  if ((field == SPH_KEY || field == SPH_CELLSTART || field == SPH_ACC || field == SPH_DRHODT ||
-       field == SPH_NBCOUNT) && ctx->n_nl == 0)
-    return fail(ctx, SPH_E_STATE, "field needs a neighbour-list build / interaction pass first");
+  if ((field == SPH_KEY || field == SPH_CELLSTART) && !ctx->has_build)
+    return fail(ctx, SPH_E_STATE, "field needs a neighbour-list build since the last load");
+  if ((field == SPH_ACC || field == SPH_DRHODT || field == SPH_NBCOUNT) && !ctx->has_pass)
+    return fail(ctx, SPH_E_STATE, "field needs an interaction pass since the last load");
   if (field == SPH_NBCOUNT && !ctx->prm.count_neighbours)
     return fail(ctx, SPH_E_STATE, "SPH_NBCOUNT needs params.count_neighbours = 1");
   if (need == 0) return SPH_OK;
@@ -592,7 +629,7 @@ SPH_EXPORT int sph_get_info(sph_ctx* ctx, sph_info* info) {
   DevScalars h;
   CK(cudaMemcpyAsync(&h, ctx->sc, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
   uint32_t nb = 0;
-  if (ctx->n_nl > 0) CK(cudaMemcpyAsync(&nb, ctx->cellstart + ctx->C.ncells, sizeof(nb), cudaMemcpyDeviceToHost, ctx->stream));
+  if (ctx->has_build) CK(cudaMemcpyAsync(&nb, ctx->cellstart + ctx->C.ncells, sizeof(nb), cudaMemcpyDeviceToHost, ctx->stream));
   CK(cudaStreamSynchronize(ctx->stream));
   memset(info, 0, sizeof(*info));
   info->n = ctx->n;
@@ -616,8 +653,7 @@ SPH_EXPORT int sph_set_profiling(sph_ctx* ctx, int32_t on) {
   if (!ctx) return SPH_E_BADARG;
   fold_events(ctx);
   if (on) {
-    for (int i = 0; i < PH_COUNT; i++) ctx->ms[i] = 0.0;
-    ctx->n_nl = ctx->n_nl;  // counters keep running; timings restart
+    for (int i = 0; i < PH_COUNT; i++) ctx->ms[i] = 0.0;   // timings restart; the counters keep running
   }
   ctx->profiling = on != 0;
   return SPH_OK;

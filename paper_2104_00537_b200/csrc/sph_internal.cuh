@@ -91,6 +91,7 @@ struct PiArgs {
   DevScalars* sc;
   int64_t n;
   uint32_t* tile_ws;           // quad kernel work space: [0] number of active tiles, [1] next tile, [4..] tile list
+  int n_sm;                    // multiprocessors of the context's device (persistent kernels: one CTA per SM)
 };
 size_t pi_quad_workspace_words(const DevConsts& C);   // size of tile_ws in 32-bit words
 void pi_gather(const DevConsts& C, const PiArgs& A, cudaStream_t s);

@@ -167,7 +167,7 @@ class Sph:
         self._h = C.c_void_p()
         rc = lib.sph_create(C.byref(sp), C.byref(self._h))
         if rc != SPH_OK:
-            raise SphError(rc, "sph_create failed")
+            raise SphError(rc, "sph_create failed: " + lib.sph_last_error(None).decode())
         self.n = 0
 
     # -- helpers ---------------------------------------------------------------------------------

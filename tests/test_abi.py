@@ -53,6 +53,27 @@ def test_bad_parameters_are_rejected_before_device_use(sph, kw):
     assert rc == sph.SPH_E_BADARG and not h.value
 
 
+def test_periodic_length_must_be_a_multiple_of_the_cell_size(sph):
+    """include/sph.h: a periodic length must be an integer multiple of the cell size (A15); otherwise particles
+    would interact across a gap.  L = 1.0 with cs = 2h = 0.0832 is not; with cell_size = L / 12 it is."""
+    h = C.c_void_p()
+    p = _params(sph)
+    p.periodic[:] = [1, 0, 0]
+    assert sph.lib.sph_create(C.byref(p), C.byref(h)) == sph.SPH_E_BADARG and not h.value
+    assert b"periodic length" in sph.lib.sph_last_error(None)
+    p.cell_size = 1.0 / 12.0
+    rc = sph.lib.sph_create(C.byref(p), C.byref(h))
+    assert rc in (sph.SPH_OK, sph.SPH_E_CUDA)      # accepted (SPH_E_CUDA on a box without a GPU)
+    if rc == sph.SPH_OK:
+        sph.lib.sph_destroy(h)
+
+
+def test_create_failure_reason_is_reported(sph):
+    h = C.c_void_p()
+    assert sph.lib.sph_create(C.byref(_params(sph, dim=4)), C.byref(h)) == sph.SPH_E_BADARG
+    assert sph.lib.sph_last_error(None) == b"dim must be 2 or 3"
+
+
 def test_null_arguments(sph):
     h = C.c_void_p()
     assert sph.lib.sph_create(None, C.byref(h)) == sph.SPH_E_BADARG

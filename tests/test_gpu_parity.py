@@ -282,8 +282,8 @@ def test_config0_ten_steps(sph, pi_kernel, cell_div):
         assert len(rho) == c.n                                           # particle count conserved (Eq. 14)
         assert abs(rho.sum() - st.rho.sum()) <= 1e-6 * st.rho.sum()
         assert_close("rho", rho, st.rho, rtol=1e-5, floor=0)
-        # velocities are not part of the stated tolerance; ten fp32 steps leave ~1e-5 |v|max of rounding
-        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-3, floor=1e-3)
+        # velocities are not part of the stated tolerance: rel 1e-4 with floor 1e-4 max|v| (tolerances: measured 6e-5 max|v| after ten steps)
+        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-4, floor=1e-4)
         # 2 builds + 2 passes per step
         tm = S.get_timings()
         assert tm.n_nl_builds == 20 and tm.n_interaction_passes == 20
@@ -317,7 +317,7 @@ def test_moving_boundary_piston(sph, pi_kernel):
         mv = c.ptype >= 2
         assert mv.sum() > 0
         assert np.abs(pos[mv, 0] - c.pos[mv, 0]).min() > 1e-5          # the piston moved
-        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-3, floor=1e-3)
+        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-4, floor=1e-4)
 
 
 def test_read_buffer_too_small_and_state_errors(sph):
@@ -370,7 +370,7 @@ def test_config0_verlet_steps(sph, verlet_steps):
         rho = S.read_state(sph.SPH_RHO).astype(np.float64)
         assert abs(rho.sum() - st.rho.sum()) <= 1e-6 * st.rho.sum()
         assert_close("rho", rho, st.rho, rtol=1e-5, floor=0)
-        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-3, floor=1e-3)
+        assert_close("vel", S.read_state(sph.SPH_VEL), st.vel, rtol=1e-4, floor=1e-4)
         tm = S.get_timings()
         assert tm.n_nl_builds == 12 and tm.n_interaction_passes == 12      # one pass per step
 
