@@ -595,3 +595,96 @@ def test_c3_keys_sort_cellstart():
     sk = key[perm]
     assert np.array_equal(cellstart, np.searchsorted(sk, np.arange(2 * ncells + 2), side="left"))
     assert cellstart[ncells] == c.n_bound and cellstart[-1] == c.n
+
+
+# ---- Eq. 37: imposed boundary motion (include/sph.h sph_set_motion) -----------------------
+MOTION = dict(group=2, axis=0, stroke=0.1, period=0.05, phase=0.3)
+
+
+def _motion_closed_form(t, m=MOTION):
+    w = 2 * math.pi / m["period"]
+    return (0.5 * m["stroke"] * (math.sin(w * t + m["phase"]) - math.sin(m["phase"])),
+            0.5 * m["stroke"] * w * math.cos(w * t + m["phase"]))
+
+
+@pytest.mark.parametrize("scheme", ["symplectic", "verlet"])
+def test_motion_law_closed_form(scheme):
+    """A moving-boundary particle follows x(t) = x0 + (stroke/2)(sin(2 pi t/T + phase) - sin(phase)) and
+    v = dx/dt at the oracle's own time t after n steps, whatever the scheme; a fixed boundary particle and the
+    other axes do not move.  (Amplitude = stroke/2, angular frequency 2 pi/T, phase, evaluation time t + dt.)"""
+    p = base_params(g=(0.0, 0.0, 0.0))
+    p["domain_min"] = (-0.3, -0.3, -0.3); p["domain_max"] = (0.3, 0.3, 0.3)
+    pos = np.array([[0.01, 0.02, 0.03], [0.15, 0.1, -0.1], [-0.2, -0.2, -0.2]])
+    typ = np.array([2, 1, 3], np.uint8)          # moving group 2, fixed, group 3 without a law
+    st = oracle.State(p, pos, np.zeros((3, 3)), np.full(3, 1000.0), typ, motions=[MOTION])
+    x0 = st.pos.copy()
+    q = 2 ** -22 * oracle.grid(p)[0]
+    for n in (1, 3, 40):
+        st.step(n) if scheme == "symplectic" else st.step_verlet(n, 4)
+        d, v = _motion_closed_form(st.t)
+        np.testing.assert_allclose(st.pos[0], x0[0] + np.array([d, 0, 0]), atol=0.51 * q, rtol=0)
+        np.testing.assert_allclose(st.vel[0], [v, 0, 0], rtol=1e-13, atol=1e-15)
+        np.testing.assert_array_equal(st.pos[1:], x0[1:])
+        assert np.all(st.vel[1:] == 0.0)
+    assert st.t > 0.05 * MOTION["period"] and abs(d) > 1e-3      # a visible part of the period was covered
+    # no fluid: dt = CFL h / c0 (Eq. 35 with dt_f = infinity)
+    assert st.dt_hist[0] == pytest.approx(p["cfl"] * p["h"] / p["c0"], rel=1e-14)
+
+
+def test_motion_is_evaluated_at_the_half_step_in_the_predictor():
+    """Eq. 33-34 with Eq. 36-37 on two particles, recomputed step by step in numpy: a fluid particle at rest next
+    to a moving boundary particle.  The second pass must see the boundary particle at x(t + dt/2) with
+    v(t + dt/2): the boundary density after one step is rho^n (2 - eps)/(2 + eps) with
+    eps = -(R^{n+1/2}/rho^{n+1/2}) dt, R^{n+1/2} = rho_b (m/rho_f) (v_b - v_f).(r_b - r_f) f_ab at the half-step
+    state; evaluating the law at t or t + dt instead changes eps by ~10 %."""
+    p = base_params(g=(0.0, 0.0, 0.0), alpha=0.0, delta=0.0)
+    p["domain_min"] = (-0.3, -0.3, -0.3); p["domain_max"] = (0.3, 0.3, 0.3)
+    mot = dict(MOTION, period=0.01, phase=0.0)   # fast piston: dt is 5 % of a period
+    pos = np.array([[0.0, 0.0, 0.0], [0.035, 0.0, 0.0]])
+    typ = np.array([2, 0], np.uint8)
+    st = oracle.State(p, pos, np.zeros((2, 3)), np.full(2, 1000.0), typ, motions=[mot])
+    xb0, xf0 = st.pos[0].copy(), st.pos[1].copy()
+    m, h = 1000.0 * DP ** 3, p["h"]
+    # pass at state n: both at rest -> R = 0, F = 0; dt from Eq. 35
+    dt = p["cfl"] * h / p["c0"]
+    def law(t):
+        w = 2 * math.pi / mot["period"]
+        return 0.5 * mot["stroke"] * math.sin(w * t), 0.5 * mot["stroke"] * w * math.cos(w * t)
+    dh, vh = law(0.5 * dt)
+    rab = (xb0 + [dh, 0, 0]) - xf0                      # fluid has F = 0, v = 0: it stays
+    f = oracle.fab(3, h, float(np.linalg.norm(rab)))
+    R_half = 1000.0 * (m / 1000.0) * (vh * rab[0]) * f  # Eq. 36 at the half step (rho^{n+1/2} = rho^n as R^n = 0)
+    eps = -(R_half / 1000.0) * dt
+    st.step(1)
+    assert st.dt_hist[0] == pytest.approx(dt, rel=1e-14)
+    # rel 1e-7: the oracle's positions sit on the 2^-22 cell grid (C1), which moves r_ab by <= 1e-8 m here
+    assert st.rho[0] == pytest.approx(1000.0 * (2 - eps) / (2 + eps), rel=1e-7)
+    assert abs(eps) > 1e-4
+    # and the same R for the fluid particle by symmetry of Eq. 15 / Eq. 36 (v_ab . r_ab is symmetric)
+    assert st.rho[1] == pytest.approx(1000.0 * (2 - eps) / (2 + eps), rel=1e-7)
+    # the wrong evaluation times would be visibly different
+    for t_wrong in (0.0, dt):
+        dw, vw = law(t_wrong)
+        rw = (xb0 + [dw, 0, 0]) - xf0
+        eps_w = -(m / 1000.0 * (vw * rw[0]) * oracle.fab(3, h, float(np.linalg.norm(rw)))) * dt
+        assert abs(eps_w - eps) > 0.02 * abs(eps)
+
+
+# ---- A10: optional floor of the boundary density at rho0 -------------------------------------------------------
+@pytest.mark.parametrize("scheme", ["symplectic", "verlet"])
+def test_rho_bound_floor_clamps_boundary_particles_only(scheme):
+    """A fluid particle moving away from a boundary particle lowers both densities (Eq. 15 / 36).  With
+    rho_bound_floor = 1 the boundary particle stays exactly at rho0 while the fluid particle is untouched; without
+    it both drop."""
+    res = {}
+    for floor in (0, 1):
+        p = base_params(g=(0.0, 0.0, 0.0), alpha=0.0, delta=0.0, rho_bound_floor=floor)
+        p["domain_min"] = (-0.3, -0.3, -0.3); p["domain_max"] = (0.3, 0.3, 0.3)
+        pos = np.array([[0.0, 0.0, 0.0], [0.03, 0.0, 0.0]])
+        vel = np.array([[0.0, 0, 0], [0.5, 0, 0]])
+        st = oracle.State(p, pos, vel, np.full(2, 1000.0), np.array([1, 0], np.uint8))
+        st.step(3) if scheme == "symplectic" else st.step_verlet(3, 2)
+        res[floor] = st.rho.copy()
+    assert res[0][0] < 1000.0 - 1e-3 and res[0][1] < 1000.0 - 1e-3
+    assert res[1][0] == 1000.0                       # clamped, exactly
+    assert res[1][1] < 1000.0 - 1e-3                 # the fluid particle is not
