@@ -29,6 +29,14 @@ class OrcParams(C.Structure):
         ("visco_model", C.c_int),
         ("nu0", C.c_double),
         ("ddt_model", C.c_int),
+        ("boundary_model", C.c_int),
+        ("mdbc_slip", C.c_int),
+        ("mdbc_det_min", C.c_double),
+        ("shift_model", C.c_int),
+        ("shift_coef", C.c_double),
+        ("shift_fs_conc", C.c_double),
+        ("shift_alpha_n", C.c_double),
+        ("shift_beta_n", C.c_double),
     ]
 
 
@@ -69,6 +77,14 @@ def make_params(p: dict) -> OrcParams:
     s.visco_model = int(p.get("visco_model", 0))
     s.nu0 = float(p.get("nu0", 0.0))
     s.ddt_model = int(p.get("ddt_model", 0))
+    s.boundary_model = int(p.get("boundary_model", 0))
+    s.mdbc_slip = int(p.get("mdbc_slip", 0))
+    s.mdbc_det_min = float(p.get("mdbc_det_min", 1e-3))
+    s.shift_model = int(p.get("shift_model", 0))
+    s.shift_coef = float(p.get("shift_coef", 2.0))
+    s.shift_fs_conc = float(p.get("shift_fs_conc", 0.0))
+    s.shift_alpha_n = float(p.get("shift_alpha_n", 0.0))
+    s.shift_beta_n = float(p.get("shift_beta_n", 0.0))
     return s
 
 
@@ -164,6 +180,58 @@ def interactions(p: dict, cell, u, out, vel, rho, ptype, mode: int = 1):
     return dict(acc=acc, drho=drho, nbcount=nb, viscmax=visc.value, n_diff=ndiff.value)
 
 
+def mdbc(p: dict, cell, u, out, vel, rho, ptype, normals, vwall=None, mode: int = 1):
+    """mDBC, Eq. 38-39: returns (vel, rho, status) with the boundary entries replaced."""
+    n = cell.shape[0]
+    vel = np.ascontiguousarray(vel, np.float64).copy()
+    rho = np.ascontiguousarray(rho, np.float64).copy()
+    ptype = np.ascontiguousarray(ptype, np.uint8)
+    normals = np.ascontiguousarray(normals, np.float64)
+    status = np.zeros(n, np.uint8)
+    sp = make_params(p)
+    vw = None if vwall is None else np.ascontiguousarray(vwall, np.float64)
+    rc = lib().orc_mdbc(C.byref(sp), C.c_int64(n), _ptr(cell, C.c_int32), _ptr(u, C.c_float),
+                        _ptr(out, C.c_uint8), _ptr(vel, C.c_double), _ptr(rho, C.c_double),
+                        _ptr(ptype, C.c_uint8), _ptr(normals, C.c_double),
+                        None if vw is None else _ptr(vw, C.c_double), C.c_int(mode), _ptr(status, C.c_uint8))
+    assert rc == 0
+    return vel, rho, status
+
+
+def concentration(p: dict, cell, u, out, rho, ptype, mode: int = 1):
+    """C_a = sum_b V_b W_ab over all particles, self included (Eq. 53)."""
+    n = cell.shape[0]
+    rho = np.ascontiguousarray(rho, np.float64)
+    ptype = np.ascontiguousarray(ptype, np.uint8)
+    conc = np.zeros(n, np.float64)
+    sp = make_params(p)
+    rc = lib().orc_concentration(C.byref(sp), C.c_int64(n), _ptr(cell, C.c_int32), _ptr(u, C.c_float),
+                                 _ptr(out, C.c_uint8), _ptr(rho, C.c_double), _ptr(ptype, C.c_uint8),
+                                 C.c_int(mode), _ptr(conc, C.c_double))
+    assert rc == 0
+    return conc
+
+
+def shift_velocity(p: dict, cell, u, out, vel, rho, ptype, conc=None, mode: int = 1):
+    """Shifting velocity delta r / dt (Eq. 40-41, 53-54) and grad C of every fluid particle."""
+    n = cell.shape[0]
+    vel = np.ascontiguousarray(vel, np.float64)
+    rho = np.ascontiguousarray(rho, np.float64)
+    ptype = np.ascontiguousarray(ptype, np.uint8)
+    if conc is None:
+        conc = concentration(p, cell, u, out, rho, ptype, mode)
+    conc = np.ascontiguousarray(conc, np.float64)
+    shift = np.zeros((n, 3), np.float64)
+    gradc = np.zeros((n, 3), np.float64)
+    sp = make_params(p)
+    rc = lib().orc_shift_velocity(C.byref(sp), C.c_int64(n), _ptr(cell, C.c_int32), _ptr(u, C.c_float),
+                                  _ptr(out, C.c_uint8), _ptr(vel, C.c_double), _ptr(rho, C.c_double),
+                                  _ptr(ptype, C.c_uint8), _ptr(conc, C.c_double), C.c_int(mode),
+                                  _ptr(shift, C.c_double), _ptr(gradc, C.c_double))
+    assert rc == 0
+    return shift, gradc
+
+
 def dt(p: dict, acc, ptype, out, viscmax: float) -> float:
     n = acc.shape[0]
     sp = make_params(p)
@@ -178,7 +246,7 @@ def dt(p: dict, acc, ptype, out, viscmax: float) -> float:
 class State:
     """Oracle-side simulation state in the canonical form (C1)."""
 
-    def __init__(self, p: dict, pos, vel, rho, ptype, motions=()):
+    def __init__(self, p: dict, pos, vel, rho, ptype, motions=(), normals=None):
         self.p = dict(p)
         self.cell, self.u, self.out = canonicalize(p, pos)
         self.vel = np.ascontiguousarray(vel, np.float64).copy()
@@ -186,6 +254,7 @@ class State:
         self.ptype = np.ascontiguousarray(ptype, np.uint8).copy()
         self.pos0 = position(p, self.cell, self.u)
         self.motions = list(motions)
+        self.normals = None if normals is None else np.ascontiguousarray(normals, np.float64).copy()
         self.t = 0.0
         self.dt_hist = []
 
@@ -211,8 +280,9 @@ class State:
                             _ptr(self.u, C.c_float), _ptr(self.out, C.c_uint8),
                             _ptr(self.vel, C.c_double), _ptr(self.rho, C.c_double),
                             _ptr(self.ptype, C.c_uint8), C.c_int(nsteps), mot, C.c_int(nm),
-                            _ptr(self.pos0, C.c_double), C.byref(t), _ptr(hist, C.c_double),
-                            C.c_int(mode))
+                            _ptr(self.pos0, C.c_double),
+                            None if self.normals is None else _ptr(self.normals, C.c_double),
+                            C.byref(t), _ptr(hist, C.c_double), C.c_int(mode))
         assert rc == 0
         self.t = t.value
         self.dt_hist.extend(hist.tolist())
@@ -240,8 +310,9 @@ class State:
                                    _ptr(self.vel, C.c_double), _ptr(self.rho, C.c_double),
                                    _ptr(self.vel_m1, C.c_double), _ptr(self.rho_m1, C.c_double),
                                    _ptr(self.ptype, C.c_uint8), C.c_int(nsteps), C.c_int(verlet_steps),
-                                   C.byref(k), mot, C.c_int(nm), _ptr(self.pos0, C.c_double), C.byref(t),
-                                   _ptr(hist, C.c_double), C.c_int(mode))
+                                   C.byref(k), mot, C.c_int(nm), _ptr(self.pos0, C.c_double),
+                                   None if self.normals is None else _ptr(self.normals, C.c_double),
+                                   C.byref(t), _ptr(hist, C.c_double), C.c_int(mode))
         assert rc == 0
         self.t = t.value
         self.kstep = k.value

@@ -22,6 +22,13 @@
  * Pade density; Verlet free fall and corrective-step rule); hydrostatic column.  The Verlet density leapfrog has no
  * closed form to pin it: "parity unpinned" for that line beyond the free-fall and N_S = 1 (Euler) cases.  Everything else (absolute per-particle values on the
  * configs) is pinned only by these plus oracle-vs-GPU agreement: "parity otherwise unpinned".
+ * Imposed motion (Eq. 37): closed form x(t), v(t) and the half-step evaluation time; rho_bound_floor (A10).
+ * NEXT-3 mDBC (tests/test_oracle_next34.py): exact reproduction of linear density fields at ghost node and boundary
+ * particle on arbitrary clouds, the system against numpy.linalg.solve on a non-linear field, ghost node at twice
+ * the normal, Shepard / no-neighbour fallbacks, Shepard velocity and no-slip, brute force == cell list,
+ * "set, not integrated" in both steppers.  NEXT-4 shifting: C = 1.00049 and grad C = 0 on the full lattice, grad C
+ * against an independent numpy brute force at two free surfaces (direction, magnitude), linearity in A_s and |v|,
+ * the Eq. 54 form, and r^{n+1}(shift) - r^{n+1}(no shift) = dt s in both steppers.
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py).
  * -ffp-contract=off matters: the canonical conversions (C1) and the fp32 pair predicate
@@ -52,6 +59,14 @@ typedef struct {
   int visco_model;        /* 0: artificial viscosity, Eq. 21-22; 1: laminar viscosity, Eq. 23 (NEXT-2) */
   double nu0;             /* kinematic viscosity of Eq. 23 */
   int ddt_model;          /* 0: Molteni-Colagrossi, Eq. 18; 1: Fourtakas et al., Eq. 19-20 (NEXT-2) */
+  int boundary_model;     /* 0: DBC, Eq. 36; 1: mDBC, Eq. 38-39 (NEXT-3) */
+  int mdbc_slip;          /* 0: boundary velocity stays the imposed one; 1: no-slip, v_B = 2 v_wall - v_G (Eq. 39, A26) */
+  double mdbc_det_min;    /* smallest |det| of the corrected-gradient system that is still solved (A25) */
+  int shift_model;        /* 0: none; 1: Fickian shifting, Eq. 40-41, 53-54 (NEXT-4) */
+  double shift_coef;      /* A_s of Eq. 41 */
+  double shift_fs_conc;   /* a fluid particle with C_a below this value is treated as a free-surface particle (A29) */
+  double shift_alpha_n;   /* a_n of Eq. 54 */
+  double shift_beta_n;    /* beta_n of Eq. 54 */
 } orc_params;
 
 typedef struct {
@@ -410,6 +425,331 @@ ORC_API int orc_interactions(const orc_params* p, int64_t n, const int32_t* cell
   return 0;
 }
 
+/* ------------------------------------------------------------------------------------ */
+/* Neighbour enumeration for the NEXT-3 / NEXT-4 sums                                   */
+/* ------------------------------------------------------------------------------------ */
+
+/* The oracle's own cell list, keyed by cell only (all types mixed), as in orc_interactions mode 1. */
+typedef struct {
+  uint32_t *perm, *cellstart;
+} celllist_t;
+
+static void celllist_build(const consts_t* C, int64_t n, const int32_t* cell, const uint8_t* out, celllist_t* L) {
+  uint32_t ncells = (uint32_t)C->nc[0] * (uint32_t)C->nc[1] * (uint32_t)C->nc[2];
+  uint32_t* key = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
+  for (int64_t i = 0; i < n; i++)
+    key[i] = out[i] ? ncells
+                    : (uint32_t)cell[3 * i] + (uint32_t)C->nc[0] * ((uint32_t)cell[3 * i + 1] + (uint32_t)C->nc[1] * (uint32_t)cell[3 * i + 2]);
+  L->perm = (uint32_t*)malloc(sizeof(uint32_t) * (size_t)(n > 0 ? n : 1));
+  L->cellstart = (uint32_t*)malloc(sizeof(uint32_t) * ((size_t)ncells + 2));
+  orc_sort(n, key, ncells + 1, L->perm, L->cellstart);
+  free(key);
+}
+static void celllist_free(celllist_t* L) { free(L->perm); free(L->cellstart); }
+
+/* Calls cb(user, b, du) for every particle b != a, of any type, that is a neighbour of a by the canonical
+ * predicate C2 (the same neighbour set as the interaction pass, plus boundary-boundary pairs).
+ * du = (r_a - r_b)/cs.  mode 0: brute force; mode 1: cell list L. */
+typedef void (*pair_cb)(void* user, int64_t b, const double du[3]);
+static void each_neighbour(const consts_t* C, const orc_params* p, int64_t n, const int32_t* cell, const float* u,
+                           const uint8_t* out, int mode, const celllist_t* L, int64_t a, pair_cb cb, void* user) {
+  const int K = C->k;
+  const float* ua = u + 3 * a;
+  const int32_t* ca = cell + 3 * a;
+  if (mode == 0) {
+    for (int64_t b = 0; b < n; b++) {
+      if (b == a || out[b]) continue;
+      int dc[3]; int far = 0;
+      for (int k = 0; k < 3; k++) {
+        int d = cell[3 * b + k] - ca[k];
+        if (p->periodic[k]) {
+          int nk = C->nc[k];
+          d %= nk; if (d < 0) d += nk;
+          if (d > nk / 2) d -= nk;
+        }
+        dc[k] = d;
+        if (d > K || d < -K) far = 1;
+      }
+      if (far) continue;
+      double du[3]; int ex;
+      if (pair_predicate(C, ua, u + 3 * b, dc, du, &ex)) cb(user, b, du);
+    }
+    return;
+  }
+  const int ky = C->dim == 3 ? K : 0;
+  for (int dz = -K; dz <= K; dz++)
+    for (int dy = -ky; dy <= ky; dy++)
+      for (int dx = -K; dx <= K; dx++) {
+        int d3[3] = {dx, dy, dz}; int cc[3]; int skip = 0;
+        for (int k = 0; k < 3; k++) {
+          int c2 = ca[k] + d3[k];
+          if (p->periodic[k]) { c2 %= C->nc[k]; if (c2 < 0) c2 += C->nc[k]; }
+          else if (c2 < 0 || c2 >= C->nc[k]) skip = 1;
+          cc[k] = c2;
+        }
+        if (skip) continue;
+        uint32_t lin = (uint32_t)cc[0] + (uint32_t)C->nc[0] * ((uint32_t)cc[1] + (uint32_t)C->nc[1] * (uint32_t)cc[2]);
+        for (uint32_t j = L->cellstart[lin]; j < L->cellstart[lin + 1]; j++) {
+          int64_t b = L->perm[j];
+          if (b == a) continue;
+          double du[3]; int ex;
+          if (pair_predicate(C, ua, u + 3 * b, d3, du, &ex)) cb(user, b, du);
+        }
+      }
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* NEXT-3: modified dynamic boundary conditions, Eq. 38-39            */
+/* ------------------------------------------------------------------------------------ */
+
+/* Solve the m x m system A x = b (m <= 4) by Gaussian elimination with partial pivoting.
+ * Returns the determinant of A (0 if a pivot vanishes; x is then not set). */
+static double solve_small(int m, double A[4][4], double b[4], double x[4]) {
+  double det = 1.0;
+  for (int c = 0; c < m; c++) {
+    int piv = c;
+    for (int r = c + 1; r < m; r++) if (fabs(A[r][c]) > fabs(A[piv][c])) piv = r;
+    if (A[piv][c] == 0.0) return 0.0;
+    if (piv != c) {
+      for (int k = 0; k < m; k++) { double t = A[c][k]; A[c][k] = A[piv][k]; A[piv][k] = t; }
+      double t = b[c]; b[c] = b[piv]; b[piv] = t;
+      det = -det;
+    }
+    det *= A[c][c];
+    for (int r = c + 1; r < m; r++) {
+      double f = A[r][c] / A[c][c];
+      for (int k = c; k < m; k++) A[r][k] -= f * A[c][k];
+      b[r] -= f * b[c];
+    }
+  }
+  for (int r = m - 1; r >= 0; r--) {
+    double s = b[r];
+    for (int k = r + 1; k < m; k++) s -= A[r][k] * x[k];
+    x[r] = s / A[r][r];
+  }
+  return det;
+}
+
+/* mDBC.  For every boundary particle B (type != 0, in the grid):
+ *   ghost node  r_G = r_B + 2 n_B, n_B = the vector from the particle to the boundary interface, supplied by the
+ *               caller ("a ghost node is projected into the fluid across a boundary interface", A24);
+ *   corrected SPH approximation of Liu & Liu at r_G over the FLUID particles b within 2h of r_G:  with
+ *               d = r_b - r_G, W = W(|d|), grad_G W = -f d, V_b = m/rho_b, the unknowns (rho_G, grad rho_G) solve
+ *                 [ sum V W          sum V W d_j          ] [ rho_G      ]   [ sum m W          ]
+ *                 [ sum V grad_i W   sum V grad_i W d_j   ] [ grad_j rho ] = [ sum m grad_i W   ]
+ *               (the Taylor expansion rho_b = rho_G + grad rho_G . d, multiplied by V_b W and by V_b grad_i W and
+ *               summed; rho_b V_b = m);
+ *   Eq. 38      rho_B = rho_G + (r_B - r_G) . grad rho_G = rho_G - 2 n_B . grad rho_G;
+ *   Eq. 39      v_G = sum V v_b W / sum V W;  mdbc_slip = 1: v_B = 2 v_wall - v_G ("this velocity with the
+ *               direction reversed", generalised to a moving wall, A26); mdbc_slip = 0: v_B = v_wall.
+ * Fallbacks (the paper is silent, A25): |det| < mdbc_det_min -> Shepard value rho_B = sum m W / sum V W, no
+ * gradient; no fluid particle within 2h of the ghost node -> rho_B = rho0, v_B = v_wall.
+ * The ghost node is not a particle, so distances are evaluated in double from the canonical positions (the
+ * exact predicate |d| < 2h), with the minimum image on periodic axes.
+ * vel, rho: in/out (fluid entries read, boundary entries written).  vwall: n x 3 or NULL (= 0).
+ * status (n, may be NULL): 0 not a boundary particle / out, 1 full solve, 2 Shepard, 3 no neighbour. */
+ORC_API int orc_mdbc(const orc_params* p, int64_t n, const int32_t* cell, const float* u, const uint8_t* out,
+                     double* vel, double* rho, const uint8_t* type, const double* normals, const double* vwall,
+                     int mode, uint8_t* status) {
+  consts_t C; make_consts(p, &C);
+  const int K = C.k;
+  const int dim = C.dim, m1 = dim + 1;
+  const int ax[3] = {0, dim == 3 ? 1 : 2, 2};        /* active axes: (x, y, z) or (x, z) */
+  double* pos = (double*)malloc(sizeof(double) * 3 * (size_t)(n > 0 ? n : 1));
+  orc_position(p, n, cell, u, pos);
+  celllist_t L = {NULL, NULL};
+  if (mode == 1) celllist_build(&C, n, cell, out, &L);
+  double Lk[3];
+  for (int k = 0; k < 3; k++) Lk[k] = (double)C.nc[k] * C.cs;
+  double* rho_new = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  double* vel_new = (double*)malloc(sizeof(double) * 3 * (size_t)(n > 0 ? n : 1));
+
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t a = 0; a < n; a++) {
+    if (status) status[a] = 0;
+    rho_new[a] = rho[a];
+    for (int k = 0; k < 3; k++) vel_new[3 * a + k] = vel[3 * a + k];
+    if (type[a] == 0 || out[a]) continue;
+    double nrm[3] = {0.0, 0.0, 0.0}, vw[3] = {0.0, 0.0, 0.0};
+    for (int k = 0; k < 3; k++) {
+      if (normals) nrm[k] = normals[3 * a + k];
+      if (vwall) vw[k] = vwall[3 * a + k];
+    }
+    if (dim == 2) nrm[1] = 0.0;
+    double xg[3];
+    for (int k = 0; k < 3; k++) xg[k] = pos[3 * a + k] + 2.0 * nrm[k];
+
+    double A[4][4] = {{0}}, rhs[4] = {0}, sv[3] = {0, 0, 0};
+    uint32_t nb = 0;
+    /* candidate fluid particles: brute force, or the cells around the ghost node's cell */
+    int cg[3]; int cg_valid = 1;
+    for (int k = 0; k < 3; k++) {
+      if (dim == 2 && k == 1) { cg[k] = 0; continue; }
+      double sg = floor((xg[k] - p->domain_min[k]) / C.cs);
+      long ci = (long)sg;
+      if (p->periodic[k]) { ci %= C.nc[k]; if (ci < 0) ci += C.nc[k]; }
+      else if (ci < -K || ci >= C.nc[k] + K) cg_valid = 0;    /* farther than the stencil from every cell */
+      cg[k] = (int)ci;
+    }
+#define MDBC_PAIR(b)                                                                               \
+    do {                                                                                           \
+      if (type[b] != 0 || out[b]) break;                                                           \
+      double d[3], r2 = 0.0;                                                                       \
+      for (int k = 0; k < 3; k++) {                                                                \
+        d[k] = pos[3 * (b) + k] - xg[k];                                                           \
+        if (dim == 2 && k == 1) d[k] = 0.0;                                                        \
+        if (p->periodic[k]) d[k] -= Lk[k] * rint(d[k] / Lk[k]);                                    \
+        r2 += d[k] * d[k];                                                                         \
+      }                                                                                            \
+      if (!(r2 < C.R2exact)) break;                                                                \
+      double rr = sqrt(r2), Wb = orc_W(dim, C.h, rr), f = orc_fab(dim, C.h, rr);                   \
+      double Vb = C.m / rho[b];                                                                    \
+      double gW[3] = {-f * d[0], -f * d[1], -f * d[2]};     /* gradient w.r.t. the ghost node */   \
+      nb++;                                                                                        \
+      A[0][0] += Vb * Wb; rhs[0] += C.m * Wb;                                                      \
+      for (int j = 0; j < dim; j++) A[0][1 + j] += Vb * Wb * d[ax[j]];                             \
+      for (int i = 0; i < dim; i++) {                                                              \
+        A[1 + i][0] += Vb * gW[ax[i]]; rhs[1 + i] += C.m * gW[ax[i]];                              \
+        for (int j = 0; j < dim; j++) A[1 + i][1 + j] += Vb * gW[ax[i]] * d[ax[j]];                \
+      }                                                                                            \
+      for (int k = 0; k < 3; k++) sv[k] += Vb * vel[3 * (b) + k] * Wb;                             \
+    } while (0)
+    if (mode == 0) {
+      for (int64_t b = 0; b < n; b++) MDBC_PAIR(b);
+    } else if (cg_valid) {
+      const int ky = dim == 3 ? K : 0;
+      for (int dz = -K; dz <= K; dz++)
+        for (int dy = -ky; dy <= ky; dy++)
+          for (int dx = -K; dx <= K; dx++) {
+            int d3[3] = {dx, dy, dz}; int cc[3]; int skip = 0;
+            for (int k = 0; k < 3; k++) {
+              int c2 = cg[k] + d3[k];
+              if (p->periodic[k]) { c2 %= C.nc[k]; if (c2 < 0) c2 += C.nc[k]; }
+              else if (c2 < 0 || c2 >= C.nc[k]) skip = 1;
+              cc[k] = c2;
+            }
+            if (skip) continue;
+            uint32_t lin = (uint32_t)cc[0] + (uint32_t)C.nc[0] * ((uint32_t)cc[1] + (uint32_t)C.nc[1] * (uint32_t)cc[2]);
+            for (uint32_t j = L.cellstart[lin]; j < L.cellstart[lin + 1]; j++) { int64_t b = L.perm[j]; MDBC_PAIR(b); }
+          }
+    }
+#undef MDBC_PAIR
+    if (nb == 0 || !(A[0][0] > 0.0)) {       /* no fluid in reach of the ghost node (A25) */
+      rho_new[a] = p->rho0;
+      for (int k = 0; k < 3; k++) vel_new[3 * a + k] = vw[k];
+      if (status) status[a] = 3;
+      continue;
+    }
+    const double shep_rho = rhs[0] / A[0][0], sumVW = A[0][0];
+    double x[4] = {0, 0, 0, 0};
+    double det = solve_small(m1, A, rhs, x);
+    if (fabs(det) >= p->mdbc_det_min) {
+      double rb = x[0];
+      for (int j = 0; j < dim; j++) rb += -2.0 * nrm[ax[j]] * x[1 + j];     /* Eq. 38 */
+      rho_new[a] = rb;
+      if (status) status[a] = 1;
+    } else {
+      rho_new[a] = shep_rho;
+      if (status) status[a] = 2;
+    }
+    for (int k = 0; k < 3; k++) {
+      double vg = sv[k] / sumVW;                                             /* Eq. 39 */
+      vel_new[3 * a + k] = p->mdbc_slip == 1 ? 2.0 * vw[k] - vg : vw[k];
+    }
+    if (dim == 2) vel_new[3 * a + 1] = vw[1];
+  }
+  for (int64_t a = 0; a < n; a++) {
+    if (type[a] == 0 || out[a]) continue;
+    rho[a] = rho_new[a];
+    for (int k = 0; k < 3; k++) vel[3 * a + k] = vel_new[3 * a + k];
+  }
+  free(pos); free(rho_new); free(vel_new);
+  if (mode == 1) celllist_free(&L);
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------ */
+/* NEXT-4: particle shifting, Eq. 40-41 with Eq. 53-54 (434-442)     */
+/* ------------------------------------------------------------------------------------ */
+
+typedef struct { const consts_t* C; const double* rho; double sum; } conc_ctx;
+static void conc_cb(void* user, int64_t b, const double du[3]) {
+  conc_ctx* X = (conc_ctx*)user;
+  double r = sqrt(du[0] * du[0] + du[1] * du[1] + du[2] * du[2]) * X->C->cs;
+  X->sum += X->C->m / X->rho[b] * orc_W(X->C->dim, X->C->h, r);
+}
+
+/* Particle concentration, second half of Eq. 53: C_a = sum_{b in P} (m_b/rho_b) W_ab "computed through the sum
+ * of the smoothing kernel", for every particle a of any type, over every particle b of any type within 2h,
+ * b = a included (W(0); reading A27).  Neighbours by the canonical predicate C2. */
+ORC_API int orc_concentration(const orc_params* p, int64_t n, const int32_t* cell, const float* u,
+                              const uint8_t* out, const double* rho, const uint8_t* type, int mode, double* conc) {
+  (void)type;
+  consts_t C; make_consts(p, &C);
+  celllist_t L = {NULL, NULL};
+  if (mode == 1) celllist_build(&C, n, cell, out, &L);
+#pragma omp parallel for schedule(dynamic, 256)
+  for (int64_t a = 0; a < n; a++) {
+    conc[a] = 0.0;
+    if (out[a]) continue;
+    conc_ctx X = {&C, rho, C.m / rho[a] * orc_W(C.dim, C.h, 0.0)};
+    each_neighbour(&C, p, n, cell, u, out, mode, &L, a, conc_cb, &X);
+    conc[a] = X.sum;
+  }
+  if (mode == 1) celllist_free(&L);
+  return 0;
+}
+
+typedef struct { const consts_t* C; const double* rho; const double* conc; double Ca; double g[3]; } gradc_ctx;
+static void gradc_cb(void* user, int64_t b, const double du[3]) {
+  gradc_ctx* X = (gradc_ctx*)user;
+  const consts_t* C = X->C;
+  double r[3] = {du[0] * C->cs, du[1] * C->cs, du[2] * C->cs};
+  double f = orc_fab(C->dim, C->h, sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]));
+  double w = C->m / X->rho[b] * (X->conc[b] - X->Ca) * f;          /* V_b (C_b - C_a), grad_a W_ab = f r_ab */
+  X->g[0] += w * r[0]; X->g[1] += w * r[1]; X->g[2] += w * r[2];
+}
+
+/* Shifting velocity s_a = delta r_a / dt of every fluid particle (0 for boundary particles):
+ *   Eq. 53   grad C_a = sum_{b in P} (m_b/rho_b) (C_b - C_a) grad_a W_ab  (conc = C of orc_concentration);
+ *   Eq. 40-41  delta r_a = -D_s grad C_a,  D_s = A_s h |v_a| dt   =>  s_a = -A_s h |v_a| grad C_a;
+ *   Eq. 54   for a free-surface particle (C_a < shift_fs_conc, A29) the shift is restricted to
+ *            -D_s [ dC/ds s + dC/db b + a_n (dC/dn - beta_n) n ] with the surface normal taken along the
+ *            concentration gradient, n = -grad C_a/|grad C_a| (pointing out of the fluid, A29); the tangential
+ *            derivatives then vanish identically and dC/dn = -|grad C_a|, leaving
+ *            s_a = -A_s h |v_a| a_n (-|grad C_a| - beta_n) n.
+ * gradc (n x 3, may be NULL) receives grad C_a. */
+ORC_API int orc_shift_velocity(const orc_params* p, int64_t n, const int32_t* cell, const float* u,
+                               const uint8_t* out, const double* vel, const double* rho, const uint8_t* type,
+                               const double* conc, int mode, double* shift, double* gradc) {
+  consts_t C; make_consts(p, &C);
+  celllist_t L = {NULL, NULL};
+  if (mode == 1) celllist_build(&C, n, cell, out, &L);
+#pragma omp parallel for schedule(dynamic, 256)
+  for (int64_t a = 0; a < n; a++) {
+    shift[3 * a] = shift[3 * a + 1] = shift[3 * a + 2] = 0.0;
+    if (gradc) gradc[3 * a] = gradc[3 * a + 1] = gradc[3 * a + 2] = 0.0;
+    if (out[a] || type[a] != 0) continue;
+    gradc_ctx X = {&C, rho, conc, conc[a], {0.0, 0.0, 0.0}};
+    each_neighbour(&C, p, n, cell, u, out, mode, &L, a, gradc_cb, &X);
+    if (gradc) { gradc[3 * a] = X.g[0]; gradc[3 * a + 1] = X.g[1]; gradc[3 * a + 2] = X.g[2]; }
+    const double* v = vel + 3 * a;
+    double vmag = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    double Ds = p->shift_coef * C.h * vmag;                         /* D_s / dt, Eq. 41 */
+    if (conc[a] < p->shift_fs_conc) {                               /* Eq. 54 */
+      double gn = sqrt(X.g[0] * X.g[0] + X.g[1] * X.g[1] + X.g[2] * X.g[2]);
+      if (gn > 0.0) {
+        double fac = -Ds * p->shift_alpha_n * (-gn - p->shift_beta_n);
+        for (int k = 0; k < 3; k++) shift[3 * a + k] = fac * (-X.g[k] / gn);
+      }
+    } else {
+      for (int k = 0; k < 3; k++) shift[3 * a + k] = -Ds * X.g[k];  /* Eq. 40 */
+    }
+  }
+  if (mode == 1) celllist_free(&L);
+  return 0;
+}
+
 /* Eq. 35 with A12/A13: dt_f = min_{a in F} sqrt(h/|F_a|) (F_a incl. gravity),
  * dt_cv = h / (c0 + max_pairs |mu_ab|), dt = CFL min(dt_f, dt_cv). */
 ORC_API double orc_dt(const orc_params* p, int64_t n, const double* acc, const uint8_t* type,
@@ -434,6 +774,34 @@ static void motion_at(const orc_motion* m, double t, double* disp, double* velc)
   *velc = 0.5 * m->stroke * w * cos(w * t + m->phase);
 }
 
+/* Before an interaction pass on the state at time t_state, with boundary_model = 1: the boundary particles take
+ * their density and velocity from the ghost nodes (orc_mdbc); v_wall is the imposed velocity of the particle
+ * (the motion law at t_state for a moving group, else 0). */
+static void mdbc_before_pass(const orc_params* p, int64_t n, const int32_t* cell, const float* u, const uint8_t* out,
+                             double* vel, double* rho, const uint8_t* type, const double* normals,
+                             const orc_motion* motions, int nmotions, double t_state, int mode) {
+  if (p->boundary_model != 1) return;
+  double* vw = (double*)calloc(3 * (size_t)(n > 0 ? n : 1), sizeof(double));
+  for (int64_t a = 0; a < n; a++)
+    if (type[a] >= 2)
+      for (int j = 0; j < nmotions; j++)
+        if (motions[j].group == type[a]) {
+          double d, vv; motion_at(&motions[j], t_state, &d, &vv);
+          vw[3 * a + motions[j].axis] = vv;
+        }
+  orc_mdbc(p, n, cell, u, out, vel, rho, type, normals, vw, mode, NULL);
+  free(vw);
+}
+
+/* After the last interaction pass of a step, with shift_model = 1: shifting velocity of that state (Eq. 40-41, 53-54). */
+static void shift_after_pass(const orc_params* p, int64_t n, const int32_t* cell, const float* u, const uint8_t* out,
+                             const double* vel, const double* rho, const uint8_t* type, int mode, double* shift) {
+  double* conc = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+  orc_concentration(p, n, cell, u, out, rho, type, mode, conc);
+  orc_shift_velocity(p, n, cell, u, out, vel, rho, type, conc, mode, shift, NULL);
+  free(conc);
+}
+
 /* nsteps symplectic position-Verlet predictor-corrector steps, Eq. 33-34,
  * variable dt from the pass at state n (A8).  Positions live in the canonical (cell,u) state and are
  * re-quantised (C1) after every position update.  vel, rho are double in/out.
@@ -441,10 +809,12 @@ static void motion_at(const orc_motion* m, double t, double* disp, double* velc)
  * Returns 0; *t is advanced; dt_hist (nsteps) receives each step's dt if not NULL. */
 ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, uint8_t* out,
                      double* vel, double* rho, const uint8_t* type, int nsteps,
-                     const orc_motion* motions, int nmotions, const double* pos0,
+                     const orc_motion* motions, int nmotions, const double* pos0, const double* normals,
                      double* t, double* dt_hist, int mode) {
   int ncell[3]; double cs;
   orc_grid(p, &cs, ncell, NULL);
+  const int mdbc = p->boundary_model == 1;
+  double* shift = p->shift_model == 1 ? (double*)calloc(3 * (size_t)(n > 0 ? n : 1), sizeof(double)) : NULL;
   double* pos_n = (double*)malloc(sizeof(double) * 3 * (size_t)n);
   double* vel_n = (double*)malloc(sizeof(double) * 3 * (size_t)n);
   double* rho_n = (double*)malloc(sizeof(double) * (size_t)n);
@@ -457,6 +827,7 @@ ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, ui
     double visc;
     /* state n */
     orc_position(p, n, cell, u, pos_n);
+    mdbc_before_pass(p, n, cell, u, out, vel, rho, type, normals, motions, nmotions, *t, mode);
     memcpy(vel_n, vel, sizeof(double) * 3 * (size_t)n);
     memcpy(rho_n, rho, sizeof(double) * (size_t)n);
     orc_interactions(p, n, cell, u, out, vel, rho, type, mode, F, R, nb, &visc, NULL);   /* F^n, R^n */
@@ -481,12 +852,15 @@ ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, ui
           }
         canon1(p, ncell, cs, x, cell + 3 * a, u + 3 * a, out + a);
       }
+      if (mdbc && type[a] != 0) continue;            /* mDBC: the boundary density is not integrated (A24) */
       rho[a] = rho_n[a] + 0.5 * dt * R[a];           /* fluid and boundary alike (A11) */
       if (type[a] != 0 && p->rho_bound_floor && rho[a] < p->rho0) rho[a] = p->rho0;   /* A10 */
     }
 
     /* second pass at (r, v, rho)^{n+1/2}: neighbours rebuilt */
+    mdbc_before_pass(p, n, cell, u, out, vel, rho, type, normals, motions, nmotions, *t + 0.5 * dt, mode);
     orc_interactions(p, n, cell, u, out, vel, rho, type, mode, F, R, nb, &visc, NULL);   /* F^{n+1/2}, R^{n+1/2} */
+    if (shift) shift_after_pass(p, n, cell, u, out, vel, rho, type, mode, shift);       /* of the state n+1/2 */
 
     /* corrector: v^{n+1} = v^n + dt F^{n+1/2}; r^{n+1} = r^n + dt (v^{n+1} + v^n)/2;
      * eps = -(R^{n+1/2}/rho^{n+1/2}) dt; rho^{n+1} = rho^n (2 - eps)/(2 + eps)   (Eq. 33-34) */
@@ -497,6 +871,7 @@ ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, ui
         for (int k = 0; k < 3; k++) {
           double vn1 = vel_n[3 * a + k] + dt * F[3 * a + k];
           x[k] = pos_n[3 * a + k] + dt * 0.5 * (vn1 + vel_n[3 * a + k]);
+          if (shift) x[k] += dt * shift[3 * a + k];      /* delta r_a = -D_s grad C_a, Eq. 40-41 (A28) */
           vel[3 * a + k] = vn1;
         }
         canon1(p, ncell, cs, x, cell + 3 * a, u + 3 * a, out + a);
@@ -509,11 +884,13 @@ ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, ui
           }
         canon1(p, ncell, cs, x, cell + 3 * a, u + 3 * a, out + a);
       }
+      if (mdbc && type[a] != 0) continue;
       rho[a] = rho_n[a] * (2.0 - eps) / (2.0 + eps);
       if (type[a] != 0 && p->rho_bound_floor && rho[a] < p->rho0) rho[a] = p->rho0;
     }
     *t += dt;
   }
+  free(shift);
   free(pos_n); free(vel_n); free(rho_n); free(F); free(R); free(nb);
   return 0;
 }
@@ -531,9 +908,11 @@ ORC_API int orc_step(const orc_params* p, int64_t n, int32_t* cell, float* u, ui
 ORC_API int orc_step_verlet(const orc_params* p, int64_t n, int32_t* cell, float* u, uint8_t* out,
                             double* vel, double* rho, double* vel_m1, double* rho_m1, const uint8_t* type,
                             int nsteps, int verlet_steps, int64_t* kstep, const orc_motion* motions, int nmotions,
-                            const double* pos0, double* t, double* dt_hist, int mode) {
+                            const double* pos0, const double* normals, double* t, double* dt_hist, int mode) {
   int ncell[3]; double cs;
   orc_grid(p, &cs, ncell, NULL);
+  const int mdbc = p->boundary_model == 1;
+  double* shift = p->shift_model == 1 ? (double*)calloc(3 * (size_t)(n > 0 ? n : 1), sizeof(double)) : NULL;
   double* pos_n = (double*)malloc(sizeof(double) * 3 * (size_t)n);
   double* F = (double*)malloc(sizeof(double) * 3 * (size_t)n);
   double* R = (double*)malloc(sizeof(double) * (size_t)n);
@@ -542,7 +921,9 @@ ORC_API int orc_step_verlet(const orc_params* p, int64_t n, int32_t* cell, float
   for (int s = 0; s < nsteps; s++) {
     double visc;
     orc_position(p, n, cell, u, pos_n);
+    mdbc_before_pass(p, n, cell, u, out, vel, rho, type, normals, motions, nmotions, *t, mode);
     orc_interactions(p, n, cell, u, out, vel, rho, type, mode, F, R, nb, &visc, NULL);   /* F^n, R^n */
+    if (shift) shift_after_pass(p, n, cell, u, out, vel, rho, type, mode, shift);       /* of the state n */
     double dt = orc_dt(p, n, F, type, out, visc);
     if (dt_hist) dt_hist[s] = dt;
     const int corrective = (*kstep % verlet_steps) == 0;
@@ -553,6 +934,7 @@ ORC_API int orc_step_verlet(const orc_params* p, int64_t n, int32_t* cell, float
         for (int k = 0; k < 3; k++) {
           const double vn = vel[3 * a + k], f = F[3 * a + k];
           x[k] = pos_n[3 * a + k] + dt * vn + 0.5 * dt * dt * f;
+          if (shift) x[k] += dt * shift[3 * a + k];      /* Eq. 40-41 (A28) */
           vel[3 * a + k] = corrective ? vn + dt * f : vel_m1[3 * a + k] + 2.0 * dt * f;
           vel_m1[3 * a + k] = vn;
         }
@@ -566,13 +948,16 @@ ORC_API int orc_step_verlet(const orc_params* p, int64_t n, int32_t* cell, float
           }
         canon1(p, ncell, cs, x, cell + 3 * a, u + 3 * a, out + a);
       }
-      rho[a] = corrective ? rho_n + dt * R[a] : rho_m1[a] + 2.0 * dt * R[a];
-      if (type[a] != 0 && p->rho_bound_floor && rho[a] < p->rho0) rho[a] = p->rho0;   /* A10 */
+      if (!(mdbc && type[a] != 0)) {                 /* mDBC: the boundary density is not integrated (A24) */
+        rho[a] = corrective ? rho_n + dt * R[a] : rho_m1[a] + 2.0 * dt * R[a];
+        if (type[a] != 0 && p->rho_bound_floor && rho[a] < p->rho0) rho[a] = p->rho0;   /* A10 */
+      }
       rho_m1[a] = rho_n;
     }
     *kstep += 1;
     *t += dt;
   }
+  free(shift);
   free(pos_n); free(F); free(R); free(nb);
   return 0;
 }

@@ -2,8 +2,11 @@
 
 This module serves BOTH the CUDA library (through ``sph.py``) and the CPU oracle
 (through ``oracle/``) with identical inputs.  It holds none of the method's
-arithmetic: no kernel function, no equation of state, no neighbour search, no
-cell/offset conversion.  It imports neither the binding nor the oracle.
+per-step arithmetic: no kernel function, no neighbour search, no cell/offset
+conversion, no interaction or update formula.  The one physical recipe it holds is
+the hydrostatic initial density rho(z) = rho0 (1 + rho0 |g| depth / B)^(1/gamma) of
+the column and flume inputs (reading A18), which is input data, not a step of the
+path.  It imports neither the binding nor the oracle.
 
 Every case is a stand-in for the paper's SPHERIC Test-2 dam break
 (PAPER.md:599, section 5.3), whose case definition and data are not available here;
@@ -73,6 +76,8 @@ class Case:
     nsteps: int = 0
     motions: list = field(default_factory=list)  # dicts: group, axis, stroke, period, phase
     notes: str = ""
+    normals: np.ndarray | None = None  # (n, 3) float64, boundary particles: vector to the boundary interface (mDBC)
+    box: tuple | None = None           # ((x0, y0, z0), (x1, y1, z1)): the tank's fluid-side interface planes
 
     @property
     def n(self) -> int:
@@ -154,9 +159,30 @@ def dam_break(name, dim, dp, tank_sites, fluid_sites, jitter, seed, c0_height,
     dmin = (-m, -m if dim == 3 else 0.0, -m)
     dmax = (nx * dp + m, (ny * dp + m) if dim == 3 else 0.0, top_factor * nz * dp)
     p = _params(dim, dp, 1.2, c0, g, dmin, dmax, cell_div=cell_div)
+    lo, hi = (0.0, 0.0, 0.0), (nx * dp, ny * dp, nz * dp)
     return Case(name, np.ascontiguousarray(pos), vel, rho, ptype, p, nsteps=nsteps,
                 notes=f"dam break dim={dim} dp={dp} tank={tank_sites} fluid={fluid_sites} "
-                      f"jitter={jitter} seed={seed}")
+                      f"jitter={jitter} seed={seed}",
+                normals=box_normals(pos, ptype, lo, hi, dim=dim), box=(lo, hi))
+
+
+def box_normals(pos, ptype, lo, hi, dim=3, open_top=True):
+    """mDBC input ("a ghost node is projected into the fluid across a boundary interface"): for every
+    boundary particle, the vector from the particle to the nearest point of the box interface [lo, hi] (the planes
+    half a spacing inside the innermost boundary layer; the top is open).  Pure geometry; fluid rows are 0."""
+    pos = np.asarray(pos, np.float64)
+    nrm = np.zeros_like(pos)
+    for ax in range(3):
+        if dim == 2 and ax == 1:
+            continue
+        x = pos[:, ax]
+        below = x < lo[ax]
+        above = x > hi[ax]
+        nrm[below, ax] = lo[ax] - x[below]
+        if not (ax == 2 and open_top):
+            nrm[above, ax] = hi[ax] - x[above]
+    nrm[np.asarray(ptype) == FLUID] = 0.0
+    return nrm
 
 
 def periodic_cloud(name, n_side, dp, jitter, seed, cell_div=1, c0=None, dim=3,
