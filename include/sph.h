@@ -3,7 +3,7 @@
  * hot path of weakly compressible SPH (arxiv 2104.00537, DualSPHysics v5.0 paper) on one B200.
  *
  * Reference for every call: /root/reference/PAPER.md (cited as PAPER.md:<line>) and the readings
- * A1..A23 / canonical definitions C1..C3 listed in DESIGN.md.
+ * A1..A29 / canonical definitions C1..C3 listed in DESIGN.md.
  *
  * General conventions
  *   - Every function returns SPH_OK (0) or a negative SPH_E_* code; nothing throws or exits.
@@ -77,6 +77,23 @@ typedef struct sph_params {
   int32_t ddt_model;         /* density diffusion term: 0 Molteni-Colagrossi, Eq. 18; 1 Fourtakas et al.,   */
                              /*   Eq. 19-20 (only the dynamic part of the density difference diffuses, A23) */
   double nu0;                /* kinematic viscosity of Eq. 23                                        */
+  int32_t boundary_model;    /* 0: DBC, Eq. 36 (boundary density from the continuity equation);      */
+                             /*   1: mDBC, Eq. 38-39: before every interaction pass the */
+                             /*   density of each boundary particle is extrapolated from its ghost node    */
+                             /*   (corrected SPH gradient over the fluid particles, sph_set_boundary_normals) */
+                             /*   and is not integrated in time (A24-A25)                                   */
+  int32_t mdbc_slip;         /* mDBC velocity of a boundary particle: 0 its imposed wall velocity (0 if     */
+                             /*   fixed); 1 no-slip, v_B = 2 v_wall - v_G with v_G the Shepard sum of Eq. 39 (A26) */
+  double mdbc_det_min;       /* the corrected-gradient system is solved when |det| >= this (0 -> 1e-3),     */
+                             /*   else the Shepard density is used without gradient (A25)                   */
+  int32_t shift_model;       /* 0: none; 1: Fickian particle shifting, Eq. 40-41 with grad C of Eq. 53 and  */
+                             /*   the free-surface form Eq. 54 (A27-A29): an     */
+                             /*   extra pair of passes after the last interaction pass of a step            */
+  double shift_coef;         /* A_s of Eq. 41 ("range [1 - 6], with a value of 2 recommended"); 0 -> 2      */
+  double shift_fs_conc;      /* a fluid particle with concentration C_a below this is a free-surface        */
+                             /*   particle and follows Eq. 54 (A29); 0 disables the free-surface form       */
+  double shift_alpha_n;      /* a_n of Eq. 54 ("0 for violent flows, 0.1 for long slow flows")              */
+  double shift_beta_n;       /* beta_n of Eq. 54 (initial concentration gradient)                           */
   sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
   sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */
   void* user;                /* passed back to dev_alloc / dev_free                                  */
@@ -106,6 +123,7 @@ typedef struct sph_info {
 typedef struct sph_timings {
   double ms_key, ms_sort, ms_cellstart, ms_reorder, ms_interaction, ms_dt, ms_update;
   int64_t n_nl_builds, n_interaction_passes, n_kernel_launches;
+  double ms_mdbc, ms_shift;   /* NEXT-3 ghost-node pass, NEXT-4 concentration + shifting passes */
 } sph_timings;
 
 /* What sph_read_state copies out.  Per-particle fields come back in the caller's ORIGINAL particle
@@ -123,7 +141,9 @@ enum sph_field {
   SPH_NBCOUNT = 9,    /* uint32[n]    neighbours per particle (needs count_neighbours = 1)          */
   SPH_CELL = 10,      /* int32[n*3]   canonical cell coordinates (C1)                               */
   SPH_OFFSET = 11,    /* float[n*3]   canonical in-cell offsets u in [0,1) on the 2^-22 grid (C1)   */
-  SPH_PRESS = 12      /* float[n]     P of the last reorder (Eq. 28)                                */
+  SPH_PRESS = 12,     /* float[n]     P of the last reorder (Eq. 28)                                */
+  SPH_CONC = 13,      /* float[n]     particle concentration C_a of the last pass (Eq. 53; shift_model = 1) */
+  SPH_SHIFT = 14      /* float[n*3]   shifting velocity delta r_a / dt of the last pass (Eq. 40-41, 54); 0 for boundary */
 };
 
 /* Create a context.  Validates params, derives constants (m, B, alpha_D, eta^2, cell grid).
@@ -148,9 +168,19 @@ int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, const float* 
 int sph_set_motion(sph_ctx* ctx, int32_t group, int32_t axis, double stroke, double period,
                    double phase);
 
+/* mDBC input (boundary_model = 1): for every particle, the vector n (metres, double[n*3], original particle
+ * order; read for boundary particles only) from the particle to the boundary interface.  The ghost node of a
+ * boundary particle is r_G = r_B + 2 n ("a ghost node is projected into the fluid across a boundary interface",
+ * PAPER.md:308; the paper does not say how the interface is described, A24).  The vectors move with the particle
+ * (imposed motions are translations).  Call after sph_load_particles; without it every n = 0 (ghost node on the
+ * particle).  Copied; synchronises the stream. */
+int sph_set_boundary_normals(sph_ctx* ctx, const double* normals);
+
 /* One neighbour-list build (cell key, radix sort, cell-range table, reorder) plus one
  * particle-interaction pass (Eq. 15, 17-18 or 19-20, 21-22 or 23, 28, 36) on the current state.
- * Results: SPH_ACC, SPH_DRHODT, SPH_NBCOUNT and the dt candidates of Eq. 35. */
+ * With boundary_model = 1 the ghost-node pass (Eq. 38-39) runs between the two; with shift_model = 1 the
+ * concentration and shifting passes (Eq. 53, 40-41, 54) follow.
+ * Results: SPH_ACC, SPH_DRHODT, SPH_NBCOUNT (+ SPH_CONC, SPH_SHIFT) and the dt candidates of Eq. 35. */
 int sph_compute_interactions(sph_ctx* ctx);
 
 /* nsteps time steps with the variable dt of Eq. 35 taken from the pass at state n (A8), all on the device,
@@ -159,7 +189,8 @@ int sph_compute_interactions(sph_ctx* ctx);
  *                 build + interaction pass) + dt reduction + predictor + corrector.
  *   integrator 1: Verlet (Eq. 30-31; A21); each step = neighbour-list build + interaction
  *                 pass + dt reduction + update; step k since the last sph_load_particles uses Eq. 31 when
- *                 k mod verlet_steps == 0, else Eq. 30. */
+ *                 k mod verlet_steps == 0, else Eq. 30.
+ * shift_model = 1: r^{n+1} += dt * (shifting velocity of the state the step's last pass saw) (A28). */
 int sph_step(sph_ctx* ctx, int32_t nsteps);
 
 /* Copy one field to host memory `dst` of `dst_bytes` bytes (must be at least the field's size, else

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libsph_b200.so")
-SOURCES = ["sph_api.cu", "nl_kernels.cu", "pi_kernels.cu", "pi_tiled.cu", "pi_quad.cu", "su_kernels.cu"]
+SOURCES = ["sph_api.cu", "nl_kernels.cu", "pi_kernels.cu", "pi_tiled.cu", "pi_quad.cu", "su_kernels.cu", "bx_kernels.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # No -use_fast_math: the canonical predicate (C2) and conversions (C1) need IEEE mul/fma/div.
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -159,24 +159,7 @@ __global__ void k_cellstart(const uint32_t* __restrict__ key, int64_t n, uint32_
   cellstart[k] = (uint32_t)lo;
 }
 
-// Tait EOS, Eq. 28, evaluated without the cancellation of (rho/rho0)^gamma - 1:
-// with e = (rho - rho0)/rho0,  (1+e)^7 - 1 = e (7 + 21 e + 35 e^2 + 35 e^3 + 21 e^4 + 7 e^5 + e^6).
-__device__ __forceinline__ float eos_pressure(const DevConsts& C, float rho) {
-  float e = (rho - C.rho0) * C.inv_rho0;
-  float x;
-  if (C.gamma_is7) {
-    float p = e + 7.f;
-    p = fmaf(p, e, 21.f);
-    p = fmaf(p, e, 35.f);
-    p = fmaf(p, e, 35.f);
-    p = fmaf(p, e, 21.f);
-    p = fmaf(p, e, 7.f);
-    x = p * e;
-  } else {
-    x = expm1f(C.gamma * log1pf(e));
-  }
-  return C.Beos * x;
-}
+// (the Tait EOS, Eq. 28, lives in sph_internal.cuh: eos_pressure)
 
 // a4 (+ a7): gather every per-particle array by the sorted index; P from rho (EOS) on the way.
 __global__ void k_reorder(DevConsts C, ParticleSet src, ParticleSet dst, const uint32_t* __restrict__ idx,

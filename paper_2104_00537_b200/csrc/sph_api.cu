@@ -13,7 +13,7 @@
 
 #define SPH_EXPORT extern "C" __attribute__((visibility("default")))
 
-enum Phase { PH_KEY = 0, PH_SORT, PH_CELLSTART, PH_REORDER, PH_PI, PH_DT, PH_UPDATE, PH_COUNT };
+enum Phase { PH_KEY = 0, PH_SORT, PH_CELLSTART, PH_REORDER, PH_PI, PH_DT, PH_UPDATE, PH_MDBC, PH_SHIFT, PH_COUNT };
 
 struct EventPair {
   int phase;
@@ -41,6 +41,10 @@ struct sph_ctx {
   int key_bits = 0;
   DevScalars* sc = nullptr;
   double* pos0 = nullptr;
+  double* normals = nullptr;    // mDBC: vector to the boundary interface, original particle order (sph_set_boundary_normals)
+  double* conc = nullptr;       // shifting: concentration C_a of the last pass, sorted order
+  float4* shiftv = nullptr;     // shifting velocity of the last pass, sorted order
+  bool has_shift = false;
   bool has_moving = false;
   std::vector<Motion> motions;
   Motion* d_motions = nullptr;
@@ -171,6 +175,11 @@ int validate(const sph_params* p, std::string& why) {
   if (p->visco_model < 0 || p->visco_model > 1) return bad("visco_model must be 0 (artificial) or 1 (laminar)");
   if (p->nu0 < 0) return bad("nu0 must be >= 0");
   if (p->ddt_model < 0 || p->ddt_model > 1) return bad("ddt_model must be 0 (Molteni) or 1 (Fourtakas)");
+  if (p->boundary_model < 0 || p->boundary_model > 1) return bad("boundary_model must be 0 (DBC) or 1 (mDBC)");
+  if (p->mdbc_slip < 0 || p->mdbc_slip > 1) return bad("mdbc_slip must be 0 (wall velocity) or 1 (no-slip)");
+  if (p->mdbc_det_min < 0) return bad("mdbc_det_min must be >= 0");
+  if (p->shift_model < 0 || p->shift_model > 1) return bad("shift_model must be 0 (none) or 1 (Fickian shifting)");
+  if (p->shift_coef < 0 || p->shift_fs_conc < 0) return bad("shift_coef and shift_fs_conc must be >= 0");
   const double cs_min = 2.0 * p->h / p->cell_div;
   if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
   for (int k = 0; k < 3; k++) {
@@ -250,6 +259,18 @@ int derive(const sph_params* p, DevConsts& C, std::string& why) {
   C.c0 = p->c0;
   C.cfl = p->cfl;
   C.inv_cs = (float)(1.0 / cs);
+  C.boundary_model = p->boundary_model;
+  C.mdbc_slip = p->mdbc_slip;
+  C.mdbc_det_min = p->mdbc_det_min > 0.0 ? p->mdbc_det_min : 1e-3;
+  C.shift_model = p->shift_model;
+  C.mass = m;
+  C.aD = aD;
+  C.c_w = (float)(m * aD);
+  C.c_gw = (float)(m * Cf * cs);
+  C.shift_ds = (float)((p->shift_coef > 0.0 ? p->shift_coef : 2.0) * p->h);
+  C.shift_fs_conc = (float)p->shift_fs_conc;
+  C.shift_alpha_n = (float)p->shift_alpha_n;
+  C.shift_beta_n = (float)p->shift_beta_n;
   return SPH_OK;
 }
 
@@ -329,6 +350,30 @@ int run_pi(sph_ctx* ctx) {
   ctx->n_launch += ctx->pi_kernel == 3 ? 4 : 2;   // reset + PI kernel (+ the quad kernel's active-tile list and |F|max pass)
   ctx->n_pi += 1;
   ctx->has_pass = true;
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+// NEXT-3: ghost-node pass on the freshly sorted state, before the interaction pass.  tfrac: the state's time is
+// t + tfrac * dt (1/2 for the second pass of a symplectic step).
+int run_mdbc(sph_ctx* ctx, double tfrac) {
+  if (ctx->C.boundary_model != 1) return SPH_OK;
+  PhaseTimer t(ctx, PH_MDBC);
+  const int nm = ctx->has_moving ? (int)ctx->motions.size() : 0;
+  bx_mdbc(ctx->C, ctx->set[ctx->cur], ctx->cellstart, ctx->n, ctx->normals, ctx->d_motions, nm, ctx->sc, tfrac,
+          ctx->stream);
+  ctx->n_launch += 1;
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+// NEXT-4: concentration + shifting velocity of the state the interaction pass just saw.
+int run_shift(sph_ctx* ctx) {
+  if (ctx->C.shift_model != 1) return SPH_OK;
+  PhaseTimer t(ctx, PH_SHIFT);
+  bx_shift(ctx->C, ctx->set[ctx->cur], ctx->cellstart, ctx->n, ctx->conc, ctx->shiftv, ctx->stream);
+  ctx->n_launch += 2;
+  ctx->has_shift = true;
   CK(cudaGetLastError());
   return SPH_OK;
 }
@@ -416,8 +461,13 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
   cudaStream_t s = ctx->stream;
   // a failed (re)load leaves the context unloaded, never half-valid
   ctx->loaded = false;
-  ctx->has_build = ctx->has_pass = false;
+  ctx->has_build = ctx->has_pass = ctx->has_shift = false;
   ctx->nl_valid = false;
+  if (ctx->normals) {                         // normals belong to one particle set
+    cudaStreamSynchronize(s);
+    dfree(ctx, ctx->normals);
+    ctx->normals = nullptr;
+  }
   if (n > ctx->cap || !ctx->acc) {            // (re)allocate particle storage
     cudaStreamSynchronize(s);
     ctx->n = 0;
@@ -443,6 +493,14 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
     }
     ctx->block_hist = (uint32_t*)dalloc(ctx, sizeof(uint32_t) * nl_radix_hist_entries(cap));
     ctx->pos0 = nullptr;
+    ctx->conc = nullptr;
+    ctx->shiftv = nullptr;
+    if (ctx->C.shift_model == 1) {
+      ctx->conc = (double*)dalloc(ctx, sizeof(double) * cap);
+      ctx->shiftv = (float4*)dalloc(ctx, sizeof(float4) * cap);
+      ok = ok && ctx->conc && ctx->shiftv;
+      if (ok) cudaMemsetAsync(ctx->shiftv, 0, sizeof(float4) * cap, s);
+    }
     ok = ok && ctx->acc && ctx->nbcount && ctx->key[0] && ctx->key[1] && ctx->idx[0] && ctx->idx[1] && ctx->block_hist;
     if (!ok) return fail(ctx, SPH_E_NOMEM, "device allocation failed for %s particles", std::to_string(n).c_str());
     ctx->cap = cap;
@@ -502,13 +560,29 @@ SPH_EXPORT int sph_set_motion(sph_ctx* ctx, int32_t group, int32_t axis, double 
   return SPH_OK;
 }
 
+SPH_EXPORT int sph_set_boundary_normals(sph_ctx* ctx, const double* normals) {
+  if (!ctx) return SPH_E_BADARG;
+  if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_set_boundary_normals before sph_load_particles");
+  if (!normals && ctx->n > 0) return fail(ctx, SPH_E_BADARG, "null normals array");
+  cudaStream_t s = ctx->stream;
+  if (!ctx->normals) {
+    ctx->normals = (double*)dalloc(ctx, sizeof(double) * 3 * (size_t)ctx->n);
+    if (!ctx->normals) return fail(ctx, SPH_E_NOMEM, "device allocation failed (normals)");
+  }
+  if (ctx->n > 0) CK(cudaMemcpyAsync(ctx->normals, normals, sizeof(double) * 3 * (size_t)ctx->n, cudaMemcpyHostToDevice, s));
+  CK(cudaStreamSynchronize(s));
+  return SPH_OK;
+}
+
 SPH_EXPORT int sph_compute_interactions(sph_ctx* ctx) {
   if (!ctx) return SPH_E_BADARG;
   if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_compute_interactions before sph_load_particles");
   int rc = build_nl(ctx, ctx->integrator == 1);   // Verlet: the state n-1 travels with every reorder
   if (rc != SPH_OK) return rc;
+  if ((rc = run_mdbc(ctx, 0.0)) != SPH_OK) return rc;
   rc = run_pi(ctx);
   if (rc != SPH_OK) return rc;
+  if ((rc = run_shift(ctx)) != SPH_OK) return rc;
   {
     PhaseTimer t(ctx, PH_DT);
     su_compute_dt(ctx->C, ctx->sc, ctx->stream);
@@ -526,7 +600,9 @@ SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
   for (int it = 0; it < nsteps && ctx->integrator == 1; it++) {   // Verlet, Eq. 30-31: one pass per step
     int rc;
     if ((rc = build_nl(ctx, true)) != SPH_OK) return rc;         // NL at state n; carries (v, rho)^{n-1}
+    if ((rc = run_mdbc(ctx, 0.0)) != SPH_OK) return rc;          // mDBC: boundary rho, v from the ghost nodes
     if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^n, R^n
+    if ((rc = run_shift(ctx)) != SPH_OK) return rc;              // shifting velocity of state n
     {
       PhaseTimer t(ctx, PH_DT);
       su_compute_dt(ctx->C, ctx->sc, s);                         // dt^n (Eq. 35)
@@ -535,7 +611,7 @@ SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
     {
       PhaseTimer t(ctx, PH_UPDATE);
       su_verlet(ctx->C, ctx->set[ctx->cur], ctx->acc, ctx->n, ctx->sc, ctx->d_motions, nm, ctx->pos0,
-                ctx->kstep % ctx->verlet_steps == 0, s);
+                ctx->kstep % ctx->verlet_steps == 0, ctx->C.shift_model == 1 ? ctx->shiftv : nullptr, s);
       ctx->n_launch += 2;
     }
     ctx->kstep++;
@@ -545,6 +621,7 @@ SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
   for (int it = 0; it < nsteps && ctx->integrator == 0; it++) {
     int rc;
     if ((rc = build_nl(ctx, false)) != SPH_OK) return rc;        // NL at state n
+    if ((rc = run_mdbc(ctx, 0.0)) != SPH_OK) return rc;          // mDBC: boundary rho, v from the ghost nodes
     if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^n, R^n
     {
       PhaseTimer t(ctx, PH_DT);
@@ -557,10 +634,13 @@ SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
       ctx->n_launch += 1;
     }
     if ((rc = build_nl(ctx, true)) != SPH_OK) return rc;         // NL at state n+1/2
+    if ((rc = run_mdbc(ctx, 0.5)) != SPH_OK) return rc;
     if ((rc = run_pi(ctx)) != SPH_OK) return rc;                 // F^{n+1/2}, R^{n+1/2}
+    if ((rc = run_shift(ctx)) != SPH_OK) return rc;              // shifting velocity of state n+1/2
     {
       PhaseTimer t(ctx, PH_UPDATE);
-      su_corrector(ctx->C, ctx->set[ctx->cur], ctx->acc, ctx->n, ctx->sc, ctx->d_motions, nm, ctx->pos0, s);
+      su_corrector(ctx->C, ctx->set[ctx->cur], ctx->acc, ctx->n, ctx->sc, ctx->d_motions, nm, ctx->pos0,
+                   ctx->C.shift_model == 1 ? ctx->shiftv : nullptr, s);
       ctx->n_launch += 2;
     }
     ctx->nl_valid = false;   // positions moved after the last build
@@ -578,8 +658,8 @@ SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst
   size_t need = 0;
   switch (field) {
     case SPH_POS: need = sizeof(double) * 3 * n; break;
-    case SPH_VEL: case SPH_ACC: case SPH_OFFSET: need = sizeof(float) * 3 * n; break;
-    case SPH_RHO: case SPH_DRHODT: case SPH_PRESS: need = sizeof(float) * n; break;
+    case SPH_VEL: case SPH_ACC: case SPH_OFFSET: case SPH_SHIFT: need = sizeof(float) * 3 * n; break;
+    case SPH_RHO: case SPH_DRHODT: case SPH_PRESS: case SPH_CONC: need = sizeof(float) * n; break;
     case SPH_KEY: case SPH_PERM: case SPH_NBCOUNT: need = sizeof(uint32_t) * n; break;
     case SPH_CELL: need = sizeof(int32_t) * 3 * n; break;
     case SPH_CELLSTART: need = sizeof(uint32_t) * ((size_t)ctx->nkeys + 1); break;
@@ -590,6 +670,8 @@ SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst
     return fail(ctx, SPH_E_STATE, "field needs a neighbour-list build since the last load");
   if ((field == SPH_ACC || field == SPH_DRHODT || field == SPH_NBCOUNT) && !ctx->has_pass)
     return fail(ctx, SPH_E_STATE, "field needs an interaction pass since the last load");
+  if ((field == SPH_CONC || field == SPH_SHIFT) && !ctx->has_shift)
+    return fail(ctx, SPH_E_STATE, "field needs shift_model = 1 and an interaction pass since the last load");
   if (field == SPH_NBCOUNT && !ctx->prm.count_neighbours)
     return fail(ctx, SPH_E_STATE, "SPH_NBCOUNT needs params.count_neighbours = 1");
   if (need == 0) return SPH_OK;
@@ -612,6 +694,8 @@ SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst
       case SPH_ACC: su_unsort_f4(ctx->acc, P.id, n, 3, 0, (float*)tmp, s); break;
       case SPH_DRHODT: su_unsort_f4(ctx->acc, P.id, n, 1, 3, (float*)tmp, s); break;
       case SPH_NBCOUNT: su_unsort_u32(ctx->nbcount, P.id, n, (uint32_t*)tmp, s); break;
+      case SPH_SHIFT: su_unsort_f4(ctx->shiftv, P.id, n, 3, 0, (float*)tmp, s); break;
+      case SPH_CONC: su_unsort_f64(ctx->conc, P.id, n, (float*)tmp, s); break;
     }
     ctx->n_launch += 1;
     cudaError_t e = cudaGetLastError();
@@ -673,5 +757,7 @@ SPH_EXPORT int sph_get_timings(sph_ctx* ctx, sph_timings* out) {
   out->n_nl_builds = ctx->n_nl;
   out->n_interaction_passes = ctx->n_pi;
   out->n_kernel_launches = ctx->n_launch;
+  out->ms_mdbc = ctx->ms[PH_MDBC];
+  out->ms_shift = ctx->ms[PH_SHIFT];
   return SPH_OK;
 }

@@ -35,7 +35,34 @@ struct DevConsts {
   double cs, dmin[3];
   double h, c0, cfl;
   float inv_cs;            // 1/cs (update kernel: du = dt * v / cs)
+  // NEXT-3 mDBC (Eq. 38-39) and NEXT-4 shifting (Eq. 40-41, 53-54)
+  int boundary_model, mdbc_slip, shift_model;
+  double mdbc_det_min;
+  double mass, aD;         // m = rho0 dp^d (A9), alpha_D of Eq. 11
+  float c_w;               // m alpha_D          : V_b W_ab = c_w (1/rho_b) w^4 (2q + 1)
+  float c_gw;              // m Cf cs            : V_b grad_a W_ab = c_gw (1/rho_b) w^3 du
+  float shift_ds;          // A_s h              : D_s / dt = shift_ds |v_a|   (Eq. 41)
+  float shift_fs_conc, shift_alpha_n, shift_beta_n;
 };
+
+// Tait EOS, Eq. 28, evaluated without the cancellation of (rho/rho0)^gamma - 1:
+// with e = (rho - rho0)/rho0,  (1+e)^7 - 1 = e (7 + 21 e + 35 e^2 + 35 e^3 + 21 e^4 + 7 e^5 + e^6).
+__device__ __forceinline__ float eos_pressure(const DevConsts& C, float rho) {
+  float e = (rho - C.rho0) * C.inv_rho0;
+  float x;
+  if (C.gamma_is7) {
+    float p = e + 7.f;
+    p = fmaf(p, e, 21.f);
+    p = fmaf(p, e, 35.f);
+    p = fmaf(p, e, 35.f);
+    p = fmaf(p, e, 21.f);
+    p = fmaf(p, e, 7.f);
+    x = p * e;
+  } else {
+    x = expm1f(C.gamma * log1pf(e));
+  }
+  return C.Beos * x;
+}
 
 // Device-resident scalars (one small struct in global memory).
 struct DevScalars {
@@ -54,6 +81,13 @@ struct Motion {
   int group, axis;
   double stroke, period, phase;
 };
+
+// Imposed motion of a boundary group (Eq. 37): displacement since t = 0 and velocity along the group's axis.
+__device__ __forceinline__ void motion_eval(const Motion& m, double t, double* disp, double* velc) {
+  const double w = 6.283185307179586476925286766559 / m.period;
+  *disp = 0.5 * m.stroke * (sin(w * t + m.phase) - sin(m.phase));
+  *velc = 0.5 * m.stroke * w * cos(w * t + m.phase);
+}
 
 // Particle arrays in the current (sorted) order.  Two sets; a reorder gathers set `cur` into `1-cur`.
 struct ParticleSet {
@@ -99,6 +133,15 @@ int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s);   // returns 
 int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s);    // 3-D, cell_div 1 only; 0 or -1 likewise
 void pi_reset_scalars(DevScalars* sc, cudaStream_t s);
 
+// ---- NEXT-3 mDBC and NEXT-4 shifting (bx_kernels.cu) ----
+// Ghost-node pass: density (Eq. 38), velocity (Eq. 39) and pressure (Eq. 28) of every boundary particle of the sorted
+// set P.  normals: double[n*3] in original order or NULL; wall velocities from the motion laws at sc->t + tfrac * sc->dt.
+void bx_mdbc(const DevConsts& C, const ParticleSet& P, const uint32_t* cellstart, int64_t n, const double* normals,
+             const Motion* motions, int nmotions, DevScalars* sc, double tfrac, cudaStream_t s);
+// Concentration C_a (Eq. 53) of every particle, then the shifting velocity (Eq. 40-41, 54) of every fluid particle.
+void bx_shift(const DevConsts& C, const ParticleSet& P, const uint32_t* cellstart, int64_t n, double* conc,
+              float4* shiftv, cudaStream_t s);
+
 // ---- system update (su_kernels.cu) ----
 void su_canonicalize(const DevConsts& C, const double* pos, const float* vel, const float* rho,
                      const uint8_t* type, int64_t n, const ParticleSet& P, double* pos0, DevScalars* sc,
@@ -106,14 +149,17 @@ void su_canonicalize(const DevConsts& C, const double* pos, const float* vel, co
 void su_compute_dt(const DevConsts& C, DevScalars* sc, cudaStream_t s);
 void su_predictor(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
                   const Motion* motions, int nmotions, const double* pos0, cudaStream_t s);
+// shiftv: shifting velocity of the last pass (NEXT-4) or NULL
 void su_corrector(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
-                  const Motion* motions, int nmotions, const double* pos0, cudaStream_t s);
+                  const Motion* motions, int nmotions, const double* pos0, const float4* shiftv, cudaStream_t s);
 // Verlet step, Eq. 30-31: corrective != 0 selects Eq. 31.  State n-1 lives in P.vel_n = (v^{n-1}, rho^{n-1}).
 void su_verlet(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
-               const Motion* motions, int nmotions, const double* pos0, int corrective, cudaStream_t s);
+               const Motion* motions, int nmotions, const double* pos0, int corrective, const float4* shiftv,
+               cudaStream_t s);
 // scatter sorted-order fields back to original order for sph_read_state
 void su_unsort_pos(const DevConsts& C, const ParticleSet& P, int64_t n, double* pos_out, int* cell_out,
                    float* off_out, cudaStream_t s);
 void su_unsort_f4(const float4* src, const uint32_t* id, int64_t n, int ncomp, int comp0, float* out,
                   cudaStream_t s);
 void su_unsort_u32(const uint32_t* src, const uint32_t* id, int64_t n, uint32_t* out, cudaStream_t s);
+void su_unsort_f64(const double* src, const uint32_t* id, int64_t n, float* out, cudaStream_t s);

@@ -100,12 +100,6 @@ __global__ void k_compute_dt(DevConsts C, DevScalars* sc) {
   sc->dt = C.cfl * (dtf < dtcv ? dtf : dtcv);
 }
 
-__device__ __forceinline__ void motion_eval(const Motion& m, double t, double* disp, double* velc) {
-  const double w = 6.283185307179586476925286766559 / m.period;
-  *disp = 0.5 * m.stroke * (sin(w * t + m.phase) - sin(m.phase));
-  *velc = 0.5 * m.stroke * w * cos(w * t + m.phase);
-}
-
 // Boundary particle with imposed motion (Eq. 37): position and velocity from the motion law at time t.
 __device__ __forceinline__ int moved_boundary(const DevConsts& C, const Motion* motions, int nmotions, int group,
                                               const double* pos0, uint32_t id, double t, float u[3], float v[3]) {
@@ -154,6 +148,7 @@ __global__ void k_predictor(DevConsts C, ParticleSet P, const float4* __restrict
   }
   float rho = fmaf(hdt, a.w, p.w);
   if (ty != 0 && C.rho_bound_floor) rho = fmaxf(rho, C.rho0);
+  if (ty != 0 && C.boundary_model == 1) rho = p.w;   // mDBC: set by the ghost-node pass, not integrated (A24)
   if (lin < 0) atomicAdd(&sc->n_out, 1u);
   P.posu[i] = make_float4(u[0], u[1], u[2], rho);
   P.velp[i] = v;
@@ -167,7 +162,7 @@ __global__ void k_predictor(DevConsts C, ParticleSet P, const float4* __restrict
 // P.vel_n holds (v^{n-1}, rho^{n-1}) on entry and (v^n, rho^n) on exit.  Boundary: rho only, + imposed motion.
 __global__ void k_verlet(DevConsts C, ParticleSet P, const float4* __restrict__ acc, int64_t n, DevScalars* sc,
                          const Motion* __restrict__ motions, int nmotions, const double* __restrict__ pos0,
-                         int corrective) {
+                         int corrective, const float4* __restrict__ shiftv) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int lin = P.cell[i];
@@ -185,6 +180,10 @@ __global__ void k_verlet(DevConsts C, ParticleSet P, const float4* __restrict__ 
   if (ty == 0) {
     const float s = dt * C.inv_cs, hs = 0.5f * dt * s;
     float du[3] = {fmaf(hs, a.x, s * v.x), fmaf(hs, a.y, s * v.y), fmaf(hs, a.z, s * v.z)};
+    if (shiftv) {   // delta r_a = -D_s grad C_a, Eq. 40-41 (A28)
+      const float4 sh = shiftv[i];
+      du[0] = fmaf(s, sh.x, du[0]); du[1] = fmaf(s, sh.y, du[1]); du[2] = fmaf(s, sh.z, du[2]);
+    }
     lin = advance_cell(C, lin, u, du);
     if (corrective) {
       v.x = fmaf(dt, a.x, v.x);
@@ -202,6 +201,7 @@ __global__ void k_verlet(DevConsts C, ParticleSet P, const float4* __restrict__ 
   }
   float rho = corrective ? fmaf(dt, a.w, p.w) : fmaf(2.0f * dt, a.w, m1.w);
   if (ty != 0 && C.rho_bound_floor) rho = fmaxf(rho, C.rho0);
+  if (ty != 0 && C.boundary_model == 1) rho = p.w;   // mDBC (A24)
   if (lin < 0) atomicAdd(&sc->n_out, 1u);
   P.posu[i] = make_float4(u[0], u[1], u[2], rho);
   P.velp[i] = v;
@@ -211,7 +211,8 @@ __global__ void k_verlet(DevConsts C, ParticleSet P, const float4* __restrict__ 
 // a9, corrector:  v^{n+1} = v^n + dt F^{n+1/2};  r^{n+1} = r^n + dt (v^{n+1} + v^n)/2;
 // eps = -(R^{n+1/2}/rho^{n+1/2}) dt;  rho^{n+1} = rho^n (2 - eps)/(2 + eps)       (Eq. 33-34)
 __global__ void k_corrector(DevConsts C, ParticleSet P, const float4* __restrict__ acc, int64_t n, DevScalars* sc,
-                            const Motion* __restrict__ motions, int nmotions, const double* __restrict__ pos0) {
+                            const Motion* __restrict__ motions, int nmotions, const double* __restrict__ pos0,
+                            const float4* __restrict__ shiftv) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   int lin = P.cell[i];
@@ -232,6 +233,11 @@ __global__ void k_corrector(DevConsts C, ParticleSet P, const float4* __restrict
     v.z = fmaf(dt, a.z, vn.z);
     float s = 0.5f * dt * C.inv_cs;
     float du[3] = {s * (v.x + vn.x), s * (v.y + vn.y), s * (v.z + vn.z)};
+    if (shiftv) {   // delta r_a = -D_s grad C_a, Eq. 40-41 (A28)
+      const float4 sh = shiftv[i];
+      const float sd = dt * C.inv_cs;
+      du[0] = fmaf(sd, sh.x, du[0]); du[1] = fmaf(sd, sh.y, du[1]); du[2] = fmaf(sd, sh.z, du[2]);
+    }
     u[0] = pn.x; u[1] = pn.y; u[2] = pn.z;
     lin = advance_cell(C, P.cell_n[i], u, du);
   } else if (ty >= 2 && nmotions > 0) {
@@ -242,6 +248,7 @@ __global__ void k_corrector(DevConsts C, ParticleSet P, const float4* __restrict
   float eps = -(a.w / ph.w) * dt;
   float rho = pn.w * (2.0f - eps) / (2.0f + eps);
   if (ty != 0 && C.rho_bound_floor) rho = fmaxf(rho, C.rho0);
+  if (ty != 0 && C.boundary_model == 1) rho = ph.w;  // mDBC: the value of the last ghost-node pass (A24)
   if (lin < 0) atomicAdd(&sc->n_out, 1u);
   P.posu[i] = make_float4(u[0], u[1], u[2], rho);
   P.velp[i] = v;
@@ -287,6 +294,13 @@ __global__ void k_unsort_f4(const float4* __restrict__ src, const uint32_t* __re
   for (int k = 0; k < ncomp; k++) out[(size_t)ncomp * i + k] = a[comp0 + k];
 }
 
+__global__ void k_unsort_f64(const double* __restrict__ src, const uint32_t* __restrict__ id, int64_t n,
+                             float* __restrict__ out) {
+  int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  out[id[j]] = (float)src[j];
+}
+
 __global__ void k_unsort_u32(const uint32_t* __restrict__ src, const uint32_t* __restrict__ id, int64_t n,
                              uint32_t* __restrict__ out) {
   int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -314,14 +328,15 @@ void su_predictor(const DevConsts& C, const ParticleSet& P, const float4* acc, i
 }
 
 void su_corrector(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
-                  const Motion* motions, int nmotions, const double* pos0, cudaStream_t s) {
-  if (n > 0) k_corrector<<<grid_for(n, 256), 256, 0, s>>>(C, P, acc, n, sc, motions, nmotions, pos0);
+                  const Motion* motions, int nmotions, const double* pos0, const float4* shiftv, cudaStream_t s) {
+  if (n > 0) k_corrector<<<grid_for(n, 256), 256, 0, s>>>(C, P, acc, n, sc, motions, nmotions, pos0, shiftv);
   k_advance_time<<<1, 1, 0, s>>>(sc);
 }
 
 void su_verlet(const DevConsts& C, const ParticleSet& P, const float4* acc, int64_t n, DevScalars* sc,
-               const Motion* motions, int nmotions, const double* pos0, int corrective, cudaStream_t s) {
-  if (n > 0) k_verlet<<<grid_for(n, 256), 256, 0, s>>>(C, P, acc, n, sc, motions, nmotions, pos0, corrective);
+               const Motion* motions, int nmotions, const double* pos0, int corrective, const float4* shiftv,
+               cudaStream_t s) {
+  if (n > 0) k_verlet<<<grid_for(n, 256), 256, 0, s>>>(C, P, acc, n, sc, motions, nmotions, pos0, corrective, shiftv);
   k_advance_time<<<1, 1, 0, s>>>(sc);
 }
 
@@ -340,4 +355,9 @@ void su_unsort_f4(const float4* src, const uint32_t* id, int64_t n, int ncomp, i
 void su_unsort_u32(const uint32_t* src, const uint32_t* id, int64_t n, uint32_t* out, cudaStream_t s) {
   if (n == 0) return;
   k_unsort_u32<<<grid_for(n, 256), 256, 0, s>>>(src, id, n, out);
+}
+
+void su_unsort_f64(const double* src, const uint32_t* id, int64_t n, float* out, cudaStream_t s) {
+  if (n == 0) return;
+  k_unsort_f64<<<grid_for(n, 256), 256, 0, s>>>(src, id, n, out);
 }

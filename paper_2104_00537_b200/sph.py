@@ -21,7 +21,7 @@ _ERRNAMES = {-1: "SPH_E_BADARG", -2: "SPH_E_NOMEM", -3: "SPH_E_CUDA", -4: "SPH_E
              -5: "SPH_E_OVERFLOW", -6: "SPH_E_NAN"}
 
 (SPH_POS, SPH_VEL, SPH_RHO, SPH_ACC, SPH_DRHODT, SPH_KEY, SPH_PERM, SPH_CELLSTART, SPH_NBCOUNT,
- SPH_CELL, SPH_OFFSET, SPH_PRESS) = range(1, 13)
+ SPH_CELL, SPH_OFFSET, SPH_PRESS, SPH_CONC, SPH_SHIFT) = range(1, 15)
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
@@ -48,6 +48,14 @@ class SphParams(C.Structure):
         ("visco_model", C.c_int32),
         ("ddt_model", C.c_int32),
         ("nu0", C.c_double),
+        ("boundary_model", C.c_int32),
+        ("mdbc_slip", C.c_int32),
+        ("mdbc_det_min", C.c_double),
+        ("shift_model", C.c_int32),
+        ("shift_coef", C.c_double),
+        ("shift_fs_conc", C.c_double),
+        ("shift_alpha_n", C.c_double),
+        ("shift_beta_n", C.c_double),
         ("dev_alloc", ALLOC_FN),
         ("dev_free", FREE_FN),
         ("user", C.c_void_p),
@@ -72,10 +80,11 @@ class SphTimings(C.Structure):
         ("ms_reorder", C.c_double), ("ms_interaction", C.c_double), ("ms_dt", C.c_double),
         ("ms_update", C.c_double),
         ("n_nl_builds", C.c_int64), ("n_interaction_passes", C.c_int64), ("n_kernel_launches", C.c_int64),
+        ("ms_mdbc", C.c_double), ("ms_shift", C.c_double),
     ]
 
 
-EXPORTS = ["sph_create", "sph_destroy", "sph_load_particles", "sph_set_motion",
+EXPORTS = ["sph_create", "sph_destroy", "sph_load_particles", "sph_set_motion", "sph_set_boundary_normals",
            "sph_compute_interactions", "sph_step", "sph_read_state", "sph_get_info",
            "sph_set_profiling", "sph_get_timings", "sph_last_error", "sph_version"]
 
@@ -92,6 +101,7 @@ def _load():
     L.sph_destroy.restype = None
     L.sph_load_particles.argtypes = [vp, C.c_int64, vp, vp, vp, vp]
     L.sph_set_motion.argtypes = [vp, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double]
+    L.sph_set_boundary_normals.argtypes = [vp, vp]
     L.sph_compute_interactions.argtypes = [vp]
     L.sph_step.argtypes = [vp, C.c_int32]
     L.sph_read_state.argtypes = [vp, C.c_int32, vp, C.c_size_t]
@@ -145,6 +155,10 @@ class Sph:
         sp.visco_model = int(params.get("visco_model", 0))
         sp.nu0 = float(params.get("nu0", 0.0))
         sp.ddt_model = int(params.get("ddt_model", 0))
+        for k in ("boundary_model", "mdbc_slip", "shift_model"):
+            setattr(sp, k, int(params.get(k, 0)))
+        for k in ("mdbc_det_min", "shift_coef", "shift_fs_conc", "shift_alpha_n", "shift_beta_n"):
+            setattr(sp, k, float(params.get(k, 0.0)))
         self._stream = stream if stream is not None else torch.cuda.current_stream()
         sp.cuda_stream = self._stream.cuda_stream
 
@@ -213,6 +227,11 @@ class Sph:
     def set_motion(self, group, axis, stroke, period, phase=0.0):
         self._ck(lib.sph_set_motion(self._h, group, axis, stroke, period, phase))
 
+    def set_boundary_normals(self, normals):
+        normals = np.ascontiguousarray(normals, np.float64)
+        assert normals.shape == (self.n, 3)
+        self._ck(lib.sph_set_boundary_normals(self._h, normals.ctypes.data))
+
     def compute_interactions(self):
         self._ck(lib.sph_compute_interactions(self._h))
 
@@ -225,7 +244,8 @@ class Sph:
         shapes = {SPH_POS: ((n, 3), np.float64), SPH_VEL: ((n, 3), np.float32), SPH_RHO: ((n,), np.float32),
                   SPH_ACC: ((n, 3), np.float32), SPH_DRHODT: ((n,), np.float32), SPH_KEY: ((n,), np.uint32),
                   SPH_PERM: ((n,), np.uint32), SPH_NBCOUNT: ((n,), np.uint32), SPH_CELL: ((n, 3), np.int32),
-                  SPH_OFFSET: ((n, 3), np.float32), SPH_PRESS: ((n,), np.float32)}
+                  SPH_OFFSET: ((n, 3), np.float32), SPH_PRESS: ((n,), np.float32),
+                  SPH_CONC: ((n,), np.float32), SPH_SHIFT: ((n, 3), np.float32)}
         if field == SPH_CELLSTART:
             info = self.get_info()
             shape, dt = (2 * info.ncells + 2,), np.uint32
@@ -256,3 +276,5 @@ class Sph:
         self.load_particles(case.pos, case.vel, case.rho, case.ptype)
         for m in case.motions:
             self.set_motion(m["group"], m["axis"], m["stroke"], m["period"], m["phase"])
+        if self._params.boundary_model == 1 and getattr(case, "normals", None) is not None:
+            self.set_boundary_normals(case.normals)
