@@ -235,9 +235,9 @@ def run_ours(args):
     def e2e_step():
         S.load_particles_ptr(n, h_pos.data_ptr(), h_vel.data_ptr(), h_rho.data_ptr(), h_typ.data_ptr())
         S.step(1)
-        S.read_state_ptr(sph.SPH_POS, o_pos.data_ptr(), o_pos.numel() * 8)
-        S.read_state_ptr(sph.SPH_VEL, o_vel.data_ptr(), o_vel.numel() * 4)
-        S.read_state_ptr(sph.SPH_RHO, o_rho.data_ptr(), o_rho.numel() * 4)
+        S.read_fields_ptr([sph.SPH_POS, sph.SPH_VEL, sph.SPH_RHO],
+                          [o_pos.data_ptr(), o_vel.data_ptr(), o_rho.data_ptr()],
+                          [o_pos.numel() * 8, o_vel.numel() * 4, o_rho.numel() * 4])
 
     e2e_steps = max(1, min(args.steps, 5))
     e2e_step()

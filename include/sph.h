@@ -197,6 +197,12 @@ int sph_step(sph_ctx* ctx, int32_t nsteps);
  * SPH_E_OVERFLOW).  Synchronises the stream.  The other device->host crossing. */
 int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst_bytes);
 
+/* Several fields in one call ("what" names a set of fields): fields[k] goes to host memory
+ * dsts[k] of dst_bytes[k] bytes.  All arguments are checked before any work is enqueued (same error codes as
+ * sph_read_state); the gathers back to the caller's particle order and the device->host copies are enqueued
+ * together and the stream is synchronised once.  nfields = 0 is a no-op. */
+int sph_read_fields(sph_ctx* ctx, int32_t nfields, const int32_t* fields, void* const* dsts, const size_t* dst_bytes);
+
 /* Fill *info (synchronises the stream). */
 int sph_get_info(sph_ctx* ctx, sph_info* info);
 

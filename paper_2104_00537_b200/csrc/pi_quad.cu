@@ -133,7 +133,7 @@ struct PairAcc2 {
   // raw sums of the two a of a lane, kept as scalars: plain FFMA accumulate in place, whereas ptxas copies a
   // loop-carried FFMA2 destination back with two moves per sum (measured on the SASS of this kernel)
   float sx[2], sy[2], sz[2], sc[2], sd[2];
-  float visc0, visc1;
+  float visc;          // max |mu_ab| / c_mu over the accepted pairs of both a (only the maximum over all particles is used, Eq. 35)
   float nb[2];        // neighbour counts, kept as floats (exact integers)
   f2 lx, ly, lz;      // laminar viscosity sums, Eq. 23 (LAM instantiations only)
 };
@@ -209,8 +209,7 @@ __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, c
       f2_fma_acc(lam, T.dvz, A.lz);
     }
     const f2 mu = f2_mul(f2_mul(y, T.rs), inside);        // mu_ab / c_mu over accepted pairs only (Eq. 21, A12)
-    A.visc0 = fmaxf(A.visc0, fabsf(f2_lo(mu)));
-    A.visc1 = fmaxf(A.visc1, fabsf(f2_hi(mu)));
+    A.visc = fmaxf(fmaxf(A.visc, fabsf(f2_lo(mu))), fabsf(f2_hi(mu)));   // one FMNMX3
     const f2 t = f2_pack(fminf(f2_lo(y), 0.f), fminf(f2_hi(y), 0.f));   // approaching pairs only (Eq. 21)
     // (Pa + Pb) / (rho_a rho_b) = kap_a / rho_b + kap_b / rho_a
     const f2 pp = f2_fma(a.kap, f2_bc(T.inv_rho_b), T.ppb);
@@ -357,7 +356,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   acc.lx = acc.ly = acc.lz = f2_pack(0.f, 0.f);
 #pragma unroll
   for (int hh = 0; hh < 2; hh++) acc.sx[hh] = acc.sy[hh] = acc.sz[hh] = acc.sc[hh] = acc.sd[hh] = acc.nb[hh] = 0.f;
-  acc.visc0 = acc.visc1 = 0.f;
+  acc.visc = 0.f;
 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
   // term only if ddt_over_boundary, A4), then the 9 fluid rows; boundary a sweeps the fluid rows only (Eq. 36).
@@ -393,8 +392,8 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       }
       // One slot = up to 32 steps; a step tests the 8 candidates of block sw + i against the 16 a of the warp with
       // one MMA.  d0 | d1 carries the sign of D for (either a of the lane, candidate 8 (sw + i) + 2t) in bit 15 and
-      // for candidate + 1 in bit 31; two funnel shifts append them to the words of the two residue streams, so
-      // that after ne steps bit p of a word belongs to step ne - 1 - p.  The loads of QB steps are issued
+      // for candidate + 1 in bit 31; they are appended to the words of the two residue streams QB steps at a
+      // time, so that after ne steps bit p of a word belongs to step ne - 1 - p.  The loads of QB steps are issued
       // together.  Steps beyond the run read whatever follows (the test records are followed by the word lists
       // in shared memory, so the addresses stay valid); their bits are masked below.
       const int nstep = min(32, s_last - sw + 1);
@@ -407,14 +406,17 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
           unsigned bb[QB];
 #pragma unroll
           for (int i = 0; i < QB; i++) bb[i] = tq[(b0 + i) * 16];   // may run past the run (never past the lists)
+          // the sign bits of the QB steps of a batch are merged first (bits 31-28: candidate 2t + 1, bits 15-12:
+          // candidate 2t, earlier step = higher bit), so that the batches do not form one long dependency chain
+          unsigned y = 0;
 #pragma unroll
           for (int i = 0; i < QB; i++) {
             unsigned d0, d1;
             mma_m16n8k8(d0, d1, fa0, fa1, bb[i], fc0, fc1);
-            const unsigned x = d0 | d1;
-            accH = __funnelshift_l(x, accH, 1);
-            accL = __funnelshift_l(x << 16, accL, 1);
+            y += ((d0 | d1) & 0x80008000u) >> i;
           }
+          accH = __funnelshift_l(y, accH, QB);
+          accL = __funnelshift_l(y << 16, accL, QB);
         }
       }
       // keep the candidates that lie inside the run [j0, j1): step i of stream h is candidate c0 + 8 i with
@@ -510,7 +512,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     r0.sy = qsum(acc.sy[0]); r1.sy = qsum(acc.sy[1]);
     r0.sz = qsum(acc.sz[0]); r1.sz = qsum(acc.sz[1]);
     r0.sd = qsum(acc.sd[0]); r1.sd = qsum(acc.sd[1]);
-    r0.visc = qmax(acc.visc0); r1.visc = qmax(acc.visc1);
+    r0.visc = r1.visc = qmax(acc.visc);
     if (LAM) {
       r0.lx = qsum(f2_lo(acc.lx)); r1.lx = qsum(f2_hi(acc.lx));
       r0.ly = qsum(f2_lo(acc.ly)); r1.ly = qsum(f2_hi(acc.ly));

@@ -104,7 +104,11 @@ __device__ __forceinline__ void pair_eval(const DevConsts& C, const LaneA& a, co
   const float gb = w3 * inv_rho_b;
   A.sc = fmaf(gb, dot, A.sc);
   if (A_FLUID) {
-    if (DDT) A.sd = fmaf(gb, a.rho - rho_b, A.sd);
+    if (DDT) {
+      float drho = a.rho - rho_b;
+      if (C.ddt_model == 1) drho -= hydrostatic_drho(C, dux, duy, duz);   // Eq. 19-20 (A23); uniform branch
+      A.sd = fmaf(gb, drho, A.sd);
+    }
     const float rs = a.rho + rho_b;
     const float x = fast_rcp((r2u + C.eta2u) * rs);
     A.visc = fmaxf(A.visc, fabsf(dot) * x * rs);       // |mu_ab| / c_mu   (Eq. 21, A12)
@@ -113,6 +117,12 @@ __device__ __forceinline__ void pair_eval(const DevConsts& C, const LaneA& a, co
     A.sx = fmaf(coef, dux, A.sx);
     A.sy = fmaf(coef, duy, A.sy);
     A.sz = fmaf(coef, duz, A.sz);
+    if (C.visco_model == 1) {                          // Eq. 23 (A22; c_pi = 0 in this model); uniform branch
+      const float lam = w3 * r2u * x;
+      A.lx = fmaf(lam, dvx, A.lx);
+      A.ly = fmaf(lam, dvy, A.ly);
+      A.lz = fmaf(lam, dvz, A.lz);
+    }
   }
 }
 
@@ -431,7 +441,6 @@ int launch_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
 int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.k != 1) return -1;
-  if (C.visco_model != 0 || C.ddt_model != 0) return -1;   // Eq. 23 / Eq. 19-20: quad (3-D) or gather kernel
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
   if (C.dim == 3) return launch_tiled<3, 512, 4992>(C, A, s);
   return launch_tiled<2, 128, 1024>(C, A, s);

@@ -41,6 +41,8 @@ struct sph_ctx {
   int key_bits = 0;
   DevScalars* sc = nullptr;
   double* pos0 = nullptr;
+  void* stage = nullptr;        // raw inputs of sph_load_particles (kept across loads)
+  size_t stage_bytes = 0;
   double* normals = nullptr;    // mDBC: vector to the boundary interface, original particle order (sph_set_boundary_normals)
   double* conc = nullptr;       // shifting: concentration C_a of the last pass, sorted order
   float4* shiftv = nullptr;     // shifting velocity of the last pass, sorted order
@@ -475,7 +477,7 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
     ctx->nbcount = nullptr;
     ctx->block_hist = nullptr;
     for (int i = 0; i < 2; i++) { ctx->key[i] = ctx->idx[i] = nullptr; ctx->set[i] = ParticleSet(); }
-    void* keep[] = {ctx->cellstart, ctx->sc, ctx->digit_total, ctx->tile_ws, ctx->d_motions};
+    void* keep[] = {ctx->cellstart, ctx->sc, ctx->digit_total, ctx->tile_ws, ctx->d_motions, ctx->stage};
     std::vector<void*> old = ctx->allocs;
     for (void* p : old) {
       bool k = false;
@@ -505,19 +507,37 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
     if (!ok) return fail(ctx, SPH_E_NOMEM, "device allocation failed for %s particles", std::to_string(n).c_str());
     ctx->cap = cap;
   }
+  // any moving-boundary group (type >= 2)?  Eight type bytes per test (sph_set_motion may follow the load, so
+  // the start positions of such particles are kept whether or not a motion law is known yet)
   ctx->has_moving = false;
-  for (int64_t i = 0; i < n; i++)
-    if (type[i] >= 2) { ctx->has_moving = true; break; }
+  {
+    int64_t i = 0;
+    for (; i + 8 <= n && !ctx->has_moving; i += 8) {
+      uint64_t w;
+      memcpy(&w, type + i, 8);
+      ctx->has_moving = (w & 0xfefefefefefefefeull) != 0;
+    }
+    for (; i < n && !ctx->has_moving; i++) ctx->has_moving = type[i] >= 2;
+  }
   if (ctx->has_moving && !ctx->pos0) {
     ctx->pos0 = (double*)dalloc(ctx, sizeof(double) * 3 * ctx->cap);
     if (!ctx->pos0) return fail(ctx, SPH_E_NOMEM, "device allocation failed (pos0)");
   }
-  // staging buffers for the raw inputs
-  double* d_pos = (double*)dalloc(ctx, sizeof(double) * 3 * n);
-  float* d_vel = (float*)dalloc(ctx, sizeof(float) * 3 * n);
-  float* d_rho = (float*)dalloc(ctx, sizeof(float) * n);
-  uint8_t* d_type = (uint8_t*)dalloc(ctx, n);
-  if (!d_pos || !d_vel || !d_rho || !d_type) return fail(ctx, SPH_E_NOMEM, "device allocation failed (staging)");
+  // staging buffer for the raw inputs, kept for the next load: [pos | vel | rho | type], each 256-byte aligned
+  auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  const size_t o_vel = up(sizeof(double) * 3 * n), o_rho = o_vel + up(sizeof(float) * 3 * n),
+               o_type = o_rho + up(sizeof(float) * n), stage_need = o_type + up((size_t)n);
+  if (stage_need > ctx->stage_bytes) {
+    if (ctx->stage) { cudaStreamSynchronize(s); dfree(ctx, ctx->stage); }
+    ctx->stage_bytes = 0;
+    ctx->stage = dalloc(ctx, stage_need);
+    if (!ctx->stage) return fail(ctx, SPH_E_NOMEM, "device allocation failed (staging)");
+    ctx->stage_bytes = stage_need;
+  }
+  double* d_pos = (double*)ctx->stage;
+  float* d_vel = (float*)((char*)ctx->stage + o_vel);
+  float* d_rho = (float*)((char*)ctx->stage + o_rho);
+  uint8_t* d_type = (uint8_t*)ctx->stage + o_type;
   CK(cudaMemsetAsync(ctx->sc, 0, sizeof(DevScalars), s));
   if (n > 0) {
     CK(cudaMemcpyAsync(d_pos, pos, sizeof(double) * 3 * n, cudaMemcpyHostToDevice, s));
@@ -530,11 +550,7 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
                   ctx->sc, s);
   ctx->n_launch += 1;
   CK(cudaGetLastError());
-  CK(cudaStreamSynchronize(s));
-  dfree(ctx, d_pos);
-  dfree(ctx, d_vel);
-  dfree(ctx, d_rho);
-  dfree(ctx, d_type);
+  CK(cudaStreamSynchronize(s));      // the caller's buffers are free again on return
   ctx->n = n;
   ctx->loaded = true;
   ctx->kstep = 0;
@@ -649,63 +665,91 @@ SPH_EXPORT int sph_step(sph_ctx* ctx, int32_t nsteps) {
   return SPH_OK;
 }
 
-SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst_bytes) {
-  if (!ctx || !dst) return SPH_E_BADARG;
+// bytes of one field (0 for an unknown field)
+static size_t field_bytes(const sph_ctx* ctx, int32_t field) {
+  const size_t n = (size_t)ctx->n;
+  switch (field) {
+    case SPH_POS: return sizeof(double) * 3 * n;
+    case SPH_VEL: case SPH_ACC: case SPH_OFFSET: case SPH_SHIFT: return sizeof(float) * 3 * n;
+    case SPH_RHO: case SPH_DRHODT: case SPH_PRESS: case SPH_CONC: return sizeof(float) * n;
+    case SPH_KEY: case SPH_PERM: case SPH_NBCOUNT: return sizeof(uint32_t) * n;
+    case SPH_CELL: return sizeof(int32_t) * 3 * n;
+    case SPH_CELLSTART: return sizeof(uint32_t) * ((size_t)ctx->nkeys + 1);
+    default: return (size_t)-1;
+  }
+}
+
+SPH_EXPORT int sph_read_fields(sph_ctx* ctx, int32_t nfields, const int32_t* fields, void* const* dsts,
+                               const size_t* dst_bytes) {
+  if (!ctx || nfields < 0 || (nfields > 0 && (!fields || !dsts || !dst_bytes))) return SPH_E_BADARG;
   if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_read_state before sph_load_particles");
   const int64_t n = ctx->n;
   cudaStream_t s = ctx->stream;
   const ParticleSet& P = ctx->set[ctx->cur];
-  size_t need = 0;
-  switch (field) {
-    case SPH_POS: need = sizeof(double) * 3 * n; break;
-    case SPH_VEL: case SPH_ACC: case SPH_OFFSET: case SPH_SHIFT: need = sizeof(float) * 3 * n; break;
-    case SPH_RHO: case SPH_DRHODT: case SPH_PRESS: case SPH_CONC: need = sizeof(float) * n; break;
-    case SPH_KEY: case SPH_PERM: case SPH_NBCOUNT: need = sizeof(uint32_t) * n; break;
-    case SPH_CELL: need = sizeof(int32_t) * 3 * n; break;
-    case SPH_CELLSTART: need = sizeof(uint32_t) * ((size_t)ctx->nkeys + 1); break;
-    default: return fail(ctx, SPH_E_BADARG, "unknown field");
+  // every argument is checked before anything is launched
+  size_t tmp_bytes = 0;
+  for (int32_t k = 0; k < nfields; k++) {
+    const int32_t field = fields[k];
+    if (!dsts[k]) return fail(ctx, SPH_E_BADARG, "null destination");
+    const size_t need = field_bytes(ctx, field);
+    if (need == (size_t)-1) return fail(ctx, SPH_E_BADARG, "unknown field");
+    if (dst_bytes[k] < need) return fail(ctx, SPH_E_OVERFLOW, "destination buffer too small");
+    if ((field == SPH_KEY || field == SPH_CELLSTART) && !ctx->has_build)
+      return fail(ctx, SPH_E_STATE, "field needs a neighbour-list build since the last load");
+    if ((field == SPH_ACC || field == SPH_DRHODT || field == SPH_NBCOUNT) && !ctx->has_pass)
+      return fail(ctx, SPH_E_STATE, "field needs an interaction pass since the last load");
+    if ((field == SPH_CONC || field == SPH_SHIFT) && !ctx->has_shift)
+      return fail(ctx, SPH_E_STATE, "field needs shift_model = 1 and an interaction pass since the last load");
+    if (field == SPH_NBCOUNT && !ctx->prm.count_neighbours)
+      return fail(ctx, SPH_E_STATE, "SPH_NBCOUNT needs params.count_neighbours = 1");
+    if (field != SPH_KEY && field != SPH_PERM && field != SPH_CELLSTART) tmp_bytes += (need + 255) & ~(size_t)255;
   }
-  if (dst_bytes < need) return fail(ctx, SPH_E_OVERFLOW, "destination buffer too small");
-  if ((field == SPH_KEY || field == SPH_CELLSTART) && !ctx->has_build)
-    return fail(ctx, SPH_E_STATE, "field needs a neighbour-list build since the last load");
-  if ((field == SPH_ACC || field == SPH_DRHODT || field == SPH_NBCOUNT) && !ctx->has_pass)
-    return fail(ctx, SPH_E_STATE, "field needs an interaction pass since the last load");
-  if ((field == SPH_CONC || field == SPH_SHIFT) && !ctx->has_shift)
-    return fail(ctx, SPH_E_STATE, "field needs shift_model = 1 and an interaction pass since the last load");
-  if (field == SPH_NBCOUNT && !ctx->prm.count_neighbours)
-    return fail(ctx, SPH_E_STATE, "SPH_NBCOUNT needs params.count_neighbours = 1");
-  if (need == 0) return SPH_OK;
-  if (field == SPH_KEY) {
-    CK(cudaMemcpyAsync(dst, ctx->key[ctx->sorted_buf], need, cudaMemcpyDeviceToHost, s));
-  } else if (field == SPH_PERM) {
-    CK(cudaMemcpyAsync(dst, P.id, need, cudaMemcpyDeviceToHost, s));
-  } else if (field == SPH_CELLSTART) {
-    CK(cudaMemcpyAsync(dst, ctx->cellstart, need, cudaMemcpyDeviceToHost, s));
-  } else {
-    void* tmp = dalloc(ctx, need);
+  // all gathers back to the caller's particle order first, then the copies, then one synchronisation
+  char* tmp = nullptr;
+  if (tmp_bytes) {
+    tmp = (char*)dalloc(ctx, tmp_bytes);
     if (!tmp) return fail(ctx, SPH_E_NOMEM, "device allocation failed (read buffer)");
+  }
+  std::vector<void*> src((size_t)nfields, nullptr);
+  size_t off = 0;
+  for (int32_t k = 0; k < nfields; k++) {
+    const int32_t field = fields[k];
+    const size_t need = field_bytes(ctx, field);
+    if (need == 0) continue;
+    if (field == SPH_KEY) { src[k] = ctx->key[ctx->sorted_buf]; continue; }
+    if (field == SPH_PERM) { src[k] = P.id; continue; }
+    if (field == SPH_CELLSTART) { src[k] = ctx->cellstart; continue; }
+    void* t = tmp + off;
+    off += (need + 255) & ~(size_t)255;
+    src[k] = t;
     switch (field) {
-      case SPH_POS: su_unsort_pos(ctx->C, P, n, (double*)tmp, nullptr, nullptr, s); break;
-      case SPH_CELL: su_unsort_pos(ctx->C, P, n, nullptr, (int*)tmp, nullptr, s); break;
-      case SPH_OFFSET: su_unsort_pos(ctx->C, P, n, nullptr, nullptr, (float*)tmp, s); break;
-      case SPH_VEL: su_unsort_f4(P.velp, P.id, n, 3, 0, (float*)tmp, s); break;
-      case SPH_PRESS: su_unsort_f4(P.velp, P.id, n, 1, 3, (float*)tmp, s); break;
-      case SPH_RHO: su_unsort_f4(P.posu, P.id, n, 1, 3, (float*)tmp, s); break;
-      case SPH_ACC: su_unsort_f4(ctx->acc, P.id, n, 3, 0, (float*)tmp, s); break;
-      case SPH_DRHODT: su_unsort_f4(ctx->acc, P.id, n, 1, 3, (float*)tmp, s); break;
-      case SPH_NBCOUNT: su_unsort_u32(ctx->nbcount, P.id, n, (uint32_t*)tmp, s); break;
-      case SPH_SHIFT: su_unsort_f4(ctx->shiftv, P.id, n, 3, 0, (float*)tmp, s); break;
-      case SPH_CONC: su_unsort_f64(ctx->conc, P.id, n, (float*)tmp, s); break;
+      case SPH_POS: su_unsort_pos(ctx->C, P, n, (double*)t, nullptr, nullptr, s); break;
+      case SPH_CELL: su_unsort_pos(ctx->C, P, n, nullptr, (int*)t, nullptr, s); break;
+      case SPH_OFFSET: su_unsort_pos(ctx->C, P, n, nullptr, nullptr, (float*)t, s); break;
+      case SPH_VEL: su_unsort_f4(P.velp, P.id, n, 3, 0, (float*)t, s); break;
+      case SPH_PRESS: su_unsort_f4(P.velp, P.id, n, 1, 3, (float*)t, s); break;
+      case SPH_RHO: su_unsort_f4(P.posu, P.id, n, 1, 3, (float*)t, s); break;
+      case SPH_ACC: su_unsort_f4(ctx->acc, P.id, n, 3, 0, (float*)t, s); break;
+      case SPH_DRHODT: su_unsort_f4(ctx->acc, P.id, n, 1, 3, (float*)t, s); break;
+      case SPH_NBCOUNT: su_unsort_u32(ctx->nbcount, P.id, n, (uint32_t*)t, s); break;
+      case SPH_SHIFT: su_unsort_f4(ctx->shiftv, P.id, n, 3, 0, (float*)t, s); break;
+      case SPH_CONC: su_unsort_f64(ctx->conc, P.id, n, (float*)t, s); break;
     }
     ctx->n_launch += 1;
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dst, tmp, need, cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    dfree(ctx, tmp);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "sph_read_state");
   }
-  CK(cudaStreamSynchronize(s));
+  cudaError_t e = cudaGetLastError();
+  for (int32_t k = 0; k < nfields && e == cudaSuccess; k++)
+    if (src[k]) e = cudaMemcpyAsync(dsts[k], src[k], field_bytes(ctx, fields[k]), cudaMemcpyDeviceToHost, s);
+  const cudaError_t e2 = cudaStreamSynchronize(s);
+  if (e == cudaSuccess) e = e2;
+  if (tmp) dfree(ctx, tmp);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "sph_read_state");
   return SPH_OK;
+}
+
+SPH_EXPORT int sph_read_state(sph_ctx* ctx, int32_t field, void* dst, size_t dst_bytes) {
+  if (!ctx || !dst) return SPH_E_BADARG;
+  return sph_read_fields(ctx, 1, &field, &dst, &dst_bytes);
 }
 
 SPH_EXPORT int sph_get_info(sph_ctx* ctx, sph_info* info) {

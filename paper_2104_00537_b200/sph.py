@@ -85,7 +85,7 @@ class SphTimings(C.Structure):
 
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_load_particles", "sph_set_motion", "sph_set_boundary_normals",
-           "sph_compute_interactions", "sph_step", "sph_read_state", "sph_get_info",
+           "sph_compute_interactions", "sph_step", "sph_read_state", "sph_read_fields", "sph_get_info",
            "sph_set_profiling", "sph_get_timings", "sph_last_error", "sph_version"]
 
 
@@ -105,6 +105,7 @@ def _load():
     L.sph_compute_interactions.argtypes = [vp]
     L.sph_step.argtypes = [vp, C.c_int32]
     L.sph_read_state.argtypes = [vp, C.c_int32, vp, C.c_size_t]
+    L.sph_read_fields.argtypes = [vp, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     L.sph_get_info.argtypes = [vp, C.POINTER(SphInfo)]
     L.sph_set_profiling.argtypes = [vp, C.c_int32]
     L.sph_get_timings.argtypes = [vp, C.POINTER(SphTimings)]
@@ -258,6 +259,14 @@ class Sph:
 
     def read_state_ptr(self, field, ptr, nbytes):
         self._ck(lib.sph_read_state(self._h, field, ptr, nbytes))
+
+    def read_fields_ptr(self, fields, ptrs, nbytes):
+        """Several fields in one call (one synchronisation): host pointers and sizes per field."""
+        k = len(fields)
+        f = (C.c_int32 * k)(*fields)
+        d = (C.c_void_p * k)(*ptrs)
+        b = (C.c_size_t * k)(*nbytes)
+        self._ck(lib.sph_read_fields(self._h, k, f, d, b))
 
     def get_info(self) -> SphInfo:
         info = SphInfo()

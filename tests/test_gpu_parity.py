@@ -416,14 +416,17 @@ def test_laminar_viscosity_steps_and_2d(sph):
         assert S.get_info().pi_kernel == 3
         assert np.abs(S.read_state(sph.SPH_POS) - st.pos).max() <= 1e-3 * c.params["dp"]
         assert_close("rho", S.read_state(sph.SPH_RHO), st.rho, rtol=1e-5, floor=0)
-    c2 = developed_state(wl.config(1, scale=0.05), 4)      # 2-D: tiled kernel hands the laminar model to the gather kernel
+    c2 = developed_state(wl.config(1, scale=0.05), 4)      # 2-D: the tiled kernel (its default) evaluates Eq. 23 too
     c2.params.update(visco_model=1, nu0=1.0e-3)
     info = check_one_pass(sph, c2, 0)
-    assert info.pi_kernel == 1
+    assert info.pi_kernel == 2
+    c2.params.update(ddt_model=1)                          # ... and Eq. 19-20 on top
+    info = check_one_pass(sph, c2, 0)
+    assert info.pi_kernel == 2
 
 
 # ---- NEXT-2: Fourtakas density diffusion, Eq. 19-20 ----------------------------------------
-@pytest.mark.parametrize("pi_kernel", [1, 3])
+@pytest.mark.parametrize("pi_kernel", KERNELS)
 @pytest.mark.parametrize("case_name", ["dam_break", "column"])
 def test_fourtakas_ddt_one_pass(sph, case_name, pi_kernel):
     """ddt_model = 1: only the dynamic part of the density difference diffuses (A23).  The resting column with
