@@ -28,6 +28,7 @@ UNIT = "interactions/s"
 FLOPS_PER_ACCEPTED = 41.0      # per accepted ordered pair
 FLOPS_PER_CANDIDATE = 8.0      # per candidate distance test
 CAND_PER_ACCEPTED = {1: 6.45, 2: 3.73, 3: 2.75}   # (2k+1)^3 cells of size 2h/k vs the 2h sphere (k=3: clipped stencil)
+CAND_PER_ACCEPTED_2D = {1: 2.865, 2: 1.989, 3: 1.733}   # (2k+1)^2 cells of size 2h/k vs the 2h disc
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 
 
@@ -261,8 +262,9 @@ def run_ours(args):
     peaks = measured_peaks()
     sm_max = float((clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0)
     pi_ms = (tm1.ms_interaction) / max(n_pi, 1)
-    c = CAND_PER_ACCEPTED[cell_div] if info0.pi_kernel == 1 or cell_div != 1 else CAND_PER_ACCEPTED[1]
-    c = min(c, CAND_PER_ACCEPTED[1])
+    cand = CAND_PER_ACCEPTED_2D if int(case.params["dim"]) == 2 else CAND_PER_ACCEPTED
+    c = cand[cell_div] if info0.pi_kernel == 1 or cell_div != 1 else cand[1]
+    c = min(c, cand[1])
     flops_per_inter = FLOPS_PER_ACCEPTED + FLOPS_PER_CANDIDATE * c
     per_pass = inter_prof / max(n_pi, 1)
     achieved = per_pass * flops_per_inter / (pi_ms * 1e-3) / 1e12

@@ -406,6 +406,10 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
           unsigned bb[QB];
 #pragma unroll
           for (int i = 0; i < QB; i++) bb[i] = tq[(b0 + i) * 16];   // may run past the run (never past the lists)
+#ifdef Q_CHECK   // development build (SPH_NVCC_EXTRA=-DQ_CHECK): every test-record load stays inside the test records + word lists
+          if (reinterpret_cast<const unsigned char*>(tq + (b0 + QB - 1) * 16 + 1) > reinterpret_cast<const unsigned char*>(S.soff))
+            atomicOr(&A.sc->flags, 1u);
+#endif
           // the sign bits of the QB steps of a batch are merged first (bits 31-28: candidate 2t + 1, bits 15-12:
           // candidate 2t, earlier step = higher bit), so that the batches do not form one long dependency chain
           unsigned y = 0;
@@ -474,7 +478,13 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     ADDR = cur != 0u ? base - (p << 7) : dummy_addr;                                                   \
     cur &= ~(1u << (p & 31u));                                                                         \
   }
+#ifdef Q_CHECK   // development build: every popped record address is a staged record or the dummy record
+#define Q_CHECK_ADDR(ADDR) if ((ADDR) > dummy_addr || ((ADDR) & 15u)) atomicOr(&A.sc->flags, 1u);
+#else
+#define Q_CHECK_ADDR(ADDR)
+#endif
 #define Q_LOAD(ADDR, PB, VB)                                                                           \
+  Q_CHECK_ADDR(ADDR)                                                                                   \
   PB = *reinterpret_cast<const float4*>(rp + ADDR);                                                    \
   VB = *reinterpret_cast<const float4*>(rv + ADDR);
 #define Q_LOOP(DDT)                                                                                    \
@@ -500,6 +510,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     if (ddt_round) Q_LOOP(true) else Q_LOOP(false)
 #undef Q_LOOP
 #undef Q_LOAD
+#undef Q_CHECK_ADDR
 #undef Q_POP
   }
 
