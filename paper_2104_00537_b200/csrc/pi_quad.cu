@@ -39,7 +39,7 @@ constexpr int QNCELL = QS * QS * QS;      // 64 staged cells per type block
 constexpr int QNR = 2 * QNCELL;           // staged ranges: block 0 = boundary, block 1 = fluid
 constexpr int QNSEG = 2 * QT * QT * QT;   // a-segments: (block, centre cell)
 constexpr int QSLOT = 8;                  // non-empty words (32 candidates of the lane's residue each) per lane per round
-constexpr int QB = 4;                     // T-phase steps whose loads are issued together
+constexpr int QB = 8;                     // T-phase steps whose loads are issued together
 constexpr float Q_MARGIN = 0.03f;         // prefilter slack in r2u, > worst-case half-precision error
 constexpr float Q_FAR = 100.0f;           // coordinate of the dummy record (never within the support)
 
@@ -410,8 +410,8 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
           if (reinterpret_cast<const unsigned char*>(tq + (b0 + QB - 1) * 16 + 1) > reinterpret_cast<const unsigned char*>(S.soff))
             atomicOr(&A.sc->flags, 1u);
 #endif
-          // the sign bits of the QB steps of a batch are merged first (bits 31-28: candidate 2t + 1, bits 15-12:
-          // candidate 2t, earlier step = higher bit), so that the batches do not form one long dependency chain
+          // the sign bits of the QB steps of a batch are merged first (top QB bits of the upper half-word: candidate 2t + 1, of the
+          // lower half-word: candidate 2t; earlier step = higher bit), so that the batches do not form one long dependency chain
           unsigned y = 0;
 #pragma unroll
           for (int i = 0; i < QB; i++) {
