@@ -376,22 +376,25 @@ __global__ void __launch_bounds__(NT, 1) k_pi_tiled(DevConsts C, PiArgs A, int n
 
   // 2. stage particles with tile-centred coordinates: u + integer cell offset - T/2.  Exact: every value is a
   //    multiple of 2^-22 with magnitude <= 2, so all differences are exact in fp32 (C1/C2).
-  for (int r = warp; r < T::NR; r += NT / 32) {
-    const uint32_t n = S.soff[r + 1] - S.soff[r];
-    if (n == 0) continue;
+  //    One staged particle per thread and trip: its range is found by bisection of the offsets (NR is a power
+  //    of two), so that every lane is busy whatever the cell populations (about 11 particles per cell in 2-D).
+  static_assert((T::NR & (T::NR - 1)) == 0, "bisection below assumes a power of two");
+  for (uint32_t j = tid; j < total; j += NT) {
+    int r = 0;
+#pragma unroll
+    for (int step = T::NR / 2; step > 0; step >>= 1)
+      if (S.soff[r + step] <= j) r += step;         // largest r with soff[r] <= j (empty ranges are skipped over)
     const int c = r % T::NCELL;
     const float fx = (float)(c % T::SX - 1) - 0.5f * T::TX,
                 fy = DIM == 3 ? (float)((c / T::SX) % T::SY - 1) - 0.5f * T::TY : 0.f,
                 fz = (float)(c / (T::SX * T::SY) - 1) - 0.5f * T::TZ;
-    const uint32_t g0 = S.gstart[r], d0 = S.soff[r];
-    for (uint32_t i = lane; i < n; i += 32) {
-      const float4 p = A.posu[g0 + i];
-      const float4 v = A.velp[g0 + i];
-      const float x = p.x + fx, y = DIM == 3 ? p.y + fy : 0.f, z = p.z + fz;
-      S.tpos[d0 + i] = make_float4(x, y, z, fmaf(z, z, fmaf(y, y, x * x)));
-      S.vrho[d0 + i] = make_float4(v.x, v.y, v.z, p.w);
-      S.press[d0 + i] = v.w;
-    }
+    const uint32_t g = S.gstart[r] + (j - S.soff[r]);
+    const float4 p = A.posu[g];
+    const float4 v = A.velp[g];
+    const float x = p.x + fx, y = DIM == 3 ? p.y + fy : 0.f, z = p.z + fz;
+    S.tpos[j] = make_float4(x, y, z, fmaf(z, z, fmaf(y, y, x * x)));
+    S.vrho[j] = make_float4(v.x, v.y, v.z, p.w);
+    S.press[j] = v.w;
   }
   __syncthreads();
 
