@@ -113,11 +113,13 @@ def _lattice(n_sites, lo=(0, 0, 0)):
 
 
 def dam_break(name, dim, dp, tank_sites, fluid_sites, jitter, seed, c0_height,
-              cell_div=1, shuffle=False, nsteps=0, layers=2, top_factor=2.0):
+              cell_div=1, shuffle=False, nsteps=0, layers=2, top_factor=2.0, obstacle=None):
     """Dam break in a tank with `layers` DBC layers (floor + side walls, open top).
 
     dim=3: tank_sites=(nx,ny,nz), fluid block at the corner (0,0,0).
     dim=2: plane (x,z): tank_sites=(nx,1,nz), fluid_sites=(fx,1,fz); y = 0.
+    obstacle = ((i0, j0, k0), (ni, nj, nk)): a box of fixed boundary particles standing on lattice sites inside
+    the tank (an obstacle in the path of the wave, the shape of the paper's performance case).
     """
     nx, ny, nz = tank_sites
     L = layers
@@ -130,6 +132,14 @@ def dam_break(name, dim, dp, tank_sites, fluid_sites, jitter, seed, c0_height,
         inside = (outer[:, 0] >= 0) & (outer[:, 0] < nx) & (outer[:, 2] >= 0)
     bsites = outer[~inside]
     fsites = _lattice(fluid_sites)
+    if obstacle is not None:
+        (i0, j0, k0), (ni, nj, nk) = obstacle
+        osites = _lattice((ni, nj if dim == 3 else 1, nk), lo=(i0, j0 if dim == 3 else 0, k0))
+        bsites = np.concatenate([bsites, osites], axis=0)
+        in_obs = ((fsites[:, 0] >= i0) & (fsites[:, 0] < i0 + ni) & (fsites[:, 2] >= k0) & (fsites[:, 2] < k0 + nk))
+        if dim == 3:
+            in_obs &= (fsites[:, 1] >= j0) & (fsites[:, 1] < j0 + nj)
+        fsites = fsites[~in_obs]
     nb, nf = len(bsites), len(fsites)
 
     bpos = (bsites.astype(np.float64) + 0.5) * dp
@@ -372,4 +382,14 @@ def config(i: int, cell_div: int = 1, scale: float = 1.0) -> Case:
         dp = 0.00684 / scale
         return wave_flume("cfg4_wave_flume_30M", dp, 20.0, 1.0, 1.5, 0.8, seed,
                           cell_div=cell_div, nsteps=2000)
+    if i == 5:
+        # not a BASELINE.json config: config 2 with a box obstacle on the floor in the path of the wave (SURVEY.md
+        # 8(f) rank 4, "Test-2-shaped workload"; the dimensions are ours, the paper's case definition is not available)
+        dp = 0.0027 / scale
+        t = (int(round(1.6 / dp)), int(round(0.67 / dp)), int(round(0.4 / dp)))
+        f = (int(round(0.4 / dp)), int(round(0.67 / dp)), int(round(0.3 / dp)))
+        obs = ((int(round(0.9 / dp)), int(round(0.235 / dp)), 0),
+               (max(4, int(round(0.12 / dp))), max(4, int(round(0.2 / dp))), max(4, int(round(0.12 / dp)))))
+        return dam_break("cfg5_dambreak3d_obstacle", 3, dp, t, f, 0.01, seed, 0.3,
+                         cell_div=cell_div, nsteps=1000, obstacle=obs)
     raise ValueError(i)

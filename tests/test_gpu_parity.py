@@ -193,6 +193,28 @@ def test_config3_full_size_periodic_cloud(sph):
         assert np.abs(acc.sum(0)).max() <= 1e-6 * np.abs(acc).sum(0).max()
 
 
+@pytest.mark.parametrize("pi_kernel", KERNELS)
+def test_dam_break_with_obstacle(sph, pi_kernel):
+    """A box of boundary particles on the floor, touching the front of the fluid block (the shape of the paper's
+    performance case; dimensions ours): one pass on a developed state, then ten steps."""
+    c = wl.dam_break("obstacle", 3, 0.02, (40, 20, 20), (15, 20, 15), 0.01, 4321, 0.3, obstacle=((15, 6, 0), (5, 8, 6)))
+    assert c.n_bound > wl.dam_break("plain", 3, 0.02, (40, 20, 20), (15, 20, 15), 0.01, 4321, 0.3).n_bound
+    check_one_pass(sph, developed_state(c, 3), pi_kernel)
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype).step(10)
+    with sph.Sph(c.params, pi_kernel=pi_kernel) as S:
+        S.load_case(c)
+        S.step(10)
+        assert np.abs(S.read_state(sph.SPH_POS) - st.pos).max() <= 1e-3 * c.params["dp"]
+        rho = S.read_state(sph.SPH_RHO).astype(np.float64)
+        assert abs(rho.sum() - st.rho.sum()) <= 1e-6 * st.rho.sum()
+
+
+def test_config5_obstacle_workload_scaled(sph):
+    c = wl.config(5, scale=0.25)
+    info = check_one_pass(sph, developed_state(c, 2), 0)
+    assert info.pi_kernel == 3
+
+
 def _perturbed(c, seed):
     """Seeded velocity and density perturbations on a config's particles (v ~ N(0, 0.02 c0) for fluid,
     rho = rho (1 + N(0, 1e-3))): every term of Eq. 15-22 is exercised on the full-size geometry."""

@@ -88,6 +88,28 @@ def test_p4_bruteforce_equals_celllist_config0(cell_div):
     assert int(a["nbcount"][F].sum()) == 1288256 + 225331
 
 
+def test_p4_obstacle_workload_bruteforce_equals_celllist_and_site_counts():
+    """Dam break with a box obstacle (workloads.dam_break(obstacle=...)): the obstacle adds exactly its lattice sites as
+    fixed boundary particles, removes none of the fluid here (it stands in front of the block), and the oracle's two
+    neighbour searches agree on it; obstacle particles are boundary particles, so they see fluid neighbours only."""
+    base = wl.dam_break("plain", 3, 0.02, (30, 12, 12), (10, 12, 10), 0.01, 4321, 0.3)
+    c = wl.dam_break("obstacle", 3, 0.02, (30, 12, 12), (10, 12, 10), 0.01, 4321, 0.3, obstacle=((10, 4, 0), (6, 4, 5)))
+    assert c.n_bound == base.n_bound + 6 * 4 * 5 and c.n_fluid == base.n_fluid
+    st = oracle.State(c.params, c.pos, c.vel, c.rho, c.ptype)
+    a = st.interactions(mode=0)
+    b = st.interactions(mode=1)
+    assert np.array_equal(a["nbcount"], b["nbcount"])
+    np.testing.assert_allclose(a["acc"], b["acc"], rtol=1e-12, atol=1e-12)
+    obs = np.arange(base.n_bound, c.n_bound)                    # the obstacle's particles follow the tank's
+    assert (c.ptype[obs] == wl.BOUND_FIXED).all()
+    # the face touching the fluid block has fluid neighbours, the far face (0.12 m > 2h = 0.083 m away) has none
+    x = c.pos[obs, 0]
+    assert a["nbcount"][obs][x < 0.22].min() > 0 and a["nbcount"][obs][x > 0.30].max() == 0
+    # an obstacle overlapping the block displaces the fluid sites it covers
+    c2 = wl.dam_break("overlap", 3, 0.02, (30, 12, 12), (10, 12, 10), 0.01, 4321, 0.3, obstacle=((8, 4, 0), (6, 4, 5)))
+    assert c2.n_fluid == base.n_fluid - 2 * 4 * 5 and c2.n_bound == c.n_bound
+
+
 @pytest.mark.parametrize("dim,periodic,cell_div", [(3, (0, 0, 0), 1), (3, (1, 1, 1), 1),
                                                    (3, (1, 1, 1), 2), (2, (0, 0, 0), 1),
                                                    (2, (1, 0, 1), 2), (3, (0, 0, 0), 2)])
