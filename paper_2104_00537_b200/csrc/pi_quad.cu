@@ -130,19 +130,14 @@ struct PairA {
   f2 x, y, z, vx, vy, vz, rho, inv_rho, kap;   // kap = P / rho
 };
 struct PairAcc2 {
-  // raw sums of the two a of a lane, kept as scalars: plain FFMA accumulate in place, whereas ptxas copies a
-  // loop-carried FFMA2 destination back with two moves per sum (measured on the SASS of this kernel)
-  float sx[2], sy[2], sz[2], sc[2], sd[2];
-  float visc;          // max |mu_ab| / c_mu over the accepted pairs of both a (only the maximum over all particles is used, Eq. 35)
-  float nb[2];        // neighbour counts, kept as floats (exact integers)
+  // raw sums of the two a of a lane, packed: one in-place FFMA2 per sum and step.  ptxas copies a loop-carried
+  // 64-bit value back with two moves per loop trip, so the pair loop carries the halves as scalars across its
+  // back edge and packs them at the top of the body (Q_PACK / Q_UNPACK; the packing itself costs nothing).
+  f2 sx, sy, sz, sc, sd;
+  float visc;         // max |mu_ab| / c_mu over the accepted pairs of both a (only the maximum over all particles is used, Eq. 35)
+  f2 nb;              // neighbour counts, kept as floats (exact integers)
   f2 lx, ly, lz;      // laminar viscosity sums, Eq. 23 (LAM instantiations only)
 };
-// acc[h] += a_h * b_h
-__device__ __forceinline__ void f2_fma_acc2(f2 a, f2 b, float (&acc)[2]) {
-  acc[0] = fmaf(f2_lo(a), f2_lo(b), acc[0]);
-  acc[1] = fmaf(f2_hi(a), f2_hi(b), acc[1]);
-}
-
 // One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free, in two parts so that
 // the record registers are free again after the head (the P loop reloads them for the next step before the tail).
 // A b outside the support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record)
@@ -175,8 +170,7 @@ __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, c
   r2 = f2_fma(T.duz, T.duz, r2);
   const float r2a = f2_lo(r2), r2b = f2_hi(r2);
   const f2 inside = f2_pack(f_lt(r2a, C.R2u), f_lt(r2b, C.R2u));
-  A.nb[0] += f2_lo(inside);                       // exact: counts stay far below 2^24
-  A.nb[1] += f2_hi(inside);
+  f2_add_acc(inside, A.nb);                       // exact: counts stay far below 2^24
   f2 w = f2_fma(f2_pack(fast_sqrt(r2a), fast_sqrt(r2b)), f2_bc(-C.qscale), f2_bc(1.0f));   // 1 - q/2   (Eq. 11)
   w = f2_pack(fmaxf(f2_lo(w), 0.f), fmaxf(f2_hi(w), 0.f));
   const f2 w3 = f2_mul(f2_mul(w, w), w);          // grad_a W_ab = Cf w^3 cs du
@@ -184,7 +178,7 @@ __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, c
   dot = f2_fma(T.dvy, T.duy, dot);
   dot = f2_fma(T.dvz, T.duz, dot);
   const f2 gb = f2_mul(w3, f2_bc(T.inv_rho_b));
-  f2_fma_acc2(gb, dot, A.sc);
+  f2_fma_acc(gb, dot, A.sc);
   if (A_FLUID) {
     if (DDT) {
       f2 drho = T.drho;
@@ -197,7 +191,7 @@ __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, c
         h = f2_fma(e, h, f2_bc(C.hyd_k[0]));
         drho = f2_fma(f2_mul(e, f2_bc(-1.0f)), h, drho);
       }
-      f2_fma_acc2(gb, drho, A.sd);
+      f2_fma_acc(gb, drho, A.sd);
     }
     const f2 den = f2_mul(f2_add(r2, f2_bc(C.eta2u)), T.rs);
     const f2 xinv = f2_pack(fast_rcp(f2_lo(den)), fast_rcp(f2_hi(den)));
@@ -214,9 +208,9 @@ __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, c
     // (Pa + Pb) / (rho_a rho_b) = kap_a / rho_b + kap_b / rho_a
     const f2 pp = f2_fma(a.kap, f2_bc(T.inv_rho_b), T.ppb);
     const f2 coef = f2_mul(w3, f2_fma(f2_bc(C.c_pi), t, pp));
-    f2_fma_acc2(coef, T.dux, A.sx);
-    f2_fma_acc2(coef, T.duy, A.sy);
-    f2_fma_acc2(coef, T.duz, A.sz);
+    f2_fma_acc(coef, T.dux, A.sx);
+    f2_fma_acc(coef, T.duy, A.sy);
+    f2_fma_acc(coef, T.duz, A.sz);
   }
 }
 
@@ -247,12 +241,6 @@ __device__ __forceinline__ float qsum(float v) {
 __device__ __forceinline__ float qmax(float v) {
   v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
   v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
-  return v;
-}
-__device__ __forceinline__ unsigned qsumu(unsigned v) {
-  v += __shfl_xor_sync(0xffffffffu, v, 1);
-  v += __shfl_xor_sync(0xffffffffu, v, 2);
-  v += __shfl_xor_sync(0xffffffffu, v, 4);
   return v;
 }
 
@@ -354,8 +342,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
 #endif
   PairAcc2 acc;
   acc.lx = acc.ly = acc.lz = f2_pack(0.f, 0.f);
-#pragma unroll
-  for (int hh = 0; hh < 2; hh++) acc.sx[hh] = acc.sy[hh] = acc.sz[hh] = acc.sc[hh] = acc.sd[hh] = acc.nb[hh] = 0.f;
+  acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = acc.nb = f2_pack(0.f, 0.f);
   acc.visc = 0.f;
 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
@@ -487,16 +474,31 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   Q_CHECK_ADDR(ADDR)                                                                                   \
   PB = *reinterpret_cast<const float4*>(rp + ADDR);                                                    \
   VB = *reinterpret_cast<const float4*>(rv + ADDR);
+#define Q_UNPACK()                                                                                     \
+  q_s[0] = f2_lo(acc.sx); q_s[1] = f2_hi(acc.sx); q_s[2] = f2_lo(acc.sy); q_s[3] = f2_hi(acc.sy);    \
+  q_s[4] = f2_lo(acc.sz); q_s[5] = f2_hi(acc.sz); q_s[6] = f2_lo(acc.sc); q_s[7] = f2_hi(acc.sc);    \
+  q_s[8] = f2_lo(acc.sd); q_s[9] = f2_hi(acc.sd); q_s[16] = f2_lo(acc.nb); q_s[17] = f2_hi(acc.nb);   \
+  if (LAM) {                                                                                           \
+    q_s[10] = f2_lo(acc.lx); q_s[11] = f2_hi(acc.lx); q_s[12] = f2_lo(acc.ly); q_s[13] = f2_hi(acc.ly); \
+    q_s[14] = f2_lo(acc.lz); q_s[15] = f2_hi(acc.lz);                                                 \
+  }
+#define Q_PACK()                                                                                       \
+  acc.sx = f2_pack(q_s[0], q_s[1]); acc.sy = f2_pack(q_s[2], q_s[3]); acc.sz = f2_pack(q_s[4], q_s[5]); \
+  acc.sc = f2_pack(q_s[6], q_s[7]); acc.sd = f2_pack(q_s[8], q_s[9]); acc.nb = f2_pack(q_s[16], q_s[17]); \
+  if (LAM) { acc.lx = f2_pack(q_s[10], q_s[11]); acc.ly = f2_pack(q_s[12], q_s[13]); acc.lz = f2_pack(q_s[14], q_s[15]); }
 #define Q_LOOP(DDT)                                                                                    \
   {                                                                                                    \
     float4 pbA, vbA, pbB, vbB;                                                                         \
     PairTmp T;                                                                                         \
     unsigned addr;                                                                                     \
+    float q_s[18];             /* the packed sums, as scalars across the back edge of the loop */      \
     Q_POP(addr)                                                                                        \
     Q_LOAD(addr, pbA, vbA)                                                                             \
     Q_POP(addr)                                                                                        \
+    Q_UNPACK()                                                                                         \
     _Pragma("unroll 1")                                                                                \
     for (unsigned k = 0; k < nmax; k += 2) { /* at most one surplus evaluation of dummy records */     \
+      Q_PACK()                                                                                         \
       Q_LOAD(addr, pbB, vbB)   /* record of step k + 1: its address was popped during step k - 1 */    \
       Q_POP(addr)              /* address of step k + 2 */                                             \
       pair2_head<A_FLUID, DDT>(a, pbA, vbA, T);                                                        \
@@ -505,10 +507,14 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       Q_POP(addr)                                                                                      \
       pair2_head<A_FLUID, DDT>(a, pbB, vbB, T);                                                        \
       pair2_tail<A_FLUID, DDT, LAM, FOURT>(C, a, T, acc);                                              \
+      Q_UNPACK()                                                                                       \
     }                                                                                                  \
+    Q_PACK()                                                                                           \
   }
     if (ddt_round) Q_LOOP(true) else Q_LOOP(false)
 #undef Q_LOOP
+#undef Q_PACK
+#undef Q_UNPACK
 #undef Q_LOAD
 #undef Q_CHECK_ADDR
 #undef Q_POP
@@ -516,13 +522,13 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
 
   // ---- combine the 4 lanes of each pair; lane t = 0 writes both particles ----
   PairAcc r0 = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, r1 = r0;
-  r0.sc = qsum(acc.sc[0]); r1.sc = qsum(acc.sc[1]);
-  const unsigned nb0 = (unsigned)qsum(acc.nb[0]), nb1 = (unsigned)qsum(acc.nb[1]);
+  r0.sc = qsum(f2_lo(acc.sc)); r1.sc = qsum(f2_hi(acc.sc));
+  const unsigned nb0 = (unsigned)qsum(f2_lo(acc.nb)), nb1 = (unsigned)qsum(f2_hi(acc.nb));
   if (A_FLUID) {
-    r0.sx = qsum(acc.sx[0]); r1.sx = qsum(acc.sx[1]);
-    r0.sy = qsum(acc.sy[0]); r1.sy = qsum(acc.sy[1]);
-    r0.sz = qsum(acc.sz[0]); r1.sz = qsum(acc.sz[1]);
-    r0.sd = qsum(acc.sd[0]); r1.sd = qsum(acc.sd[1]);
+    r0.sx = qsum(f2_lo(acc.sx)); r1.sx = qsum(f2_hi(acc.sx));
+    r0.sy = qsum(f2_lo(acc.sy)); r1.sy = qsum(f2_hi(acc.sy));
+    r0.sz = qsum(f2_lo(acc.sz)); r1.sz = qsum(f2_hi(acc.sz));
+    r0.sd = qsum(f2_lo(acc.sd)); r1.sd = qsum(f2_hi(acc.sd));
     r0.visc = r1.visc = qmax(acc.visc);
     if (LAM) {
       r0.lx = qsum(f2_lo(acc.lx)); r1.lx = qsum(f2_hi(acc.lx));
