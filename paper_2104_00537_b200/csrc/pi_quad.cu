@@ -784,8 +784,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     if (lane == 0) gi = atomicAdd(&S.seg[0], 1u);
     gi = __shfl_sync(0xffffffffu, gi, 0);
     if (gi >= 2u * ngroups) break;
-    const int part = gi >= ngroups;                 // all units of part 0 (the larger ones) are handed out first
-    gi -= (uint32_t)part * ngroups;
+    const int part = gi & 1u;                       // the two units of a group are handed out one after the other, so
+    gi >>= 1;                                       // that neighbouring warps are in different phases (4.791 against 4.806 ms)
     int s = 0;
     while (s + 1 < QNSEG && gi >= S.seg[1 + s + 1]) s++;
     const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
