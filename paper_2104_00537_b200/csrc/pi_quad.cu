@@ -587,22 +587,27 @@ __global__ void __launch_bounds__(256) k_quad_fmax(DevConsts C, const float4* __
 
 // Active-tile list: most tiles of a dam break are air.  A tile is active if its centre cells hold a particle;
 // x-adjacent cells are adjacent keys, so one (block, cy, cz) row of centre cells is one cellstart difference.
-// ws[0] = number of active tiles, ws[1] = next tile to take (both zeroed before the launch), ws[4..] = tile ids.
+// ws[0] = number of tiles with fluid, ws[1] = next tile to take, ws[2] = number of boundary-only tiles (all zeroed
+// before the launch), ws[4..] = tile ids (fluid tiles from the front, boundary-only tiles from the back).
 __global__ void __launch_bounds__(256) k_quad_tiles(DevConsts C, const uint32_t* __restrict__ cellstart, int ntx, int nty,
                                                     int ntiles, uint32_t* ws) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= ntiles) return;
   const int ox = (t % ntx) * QT, oy = ((t / ntx) % nty) * QT, oz = (t / (ntx * nty)) * QT;
   const uint32_t w = (uint32_t)min(QT, C.nc[0] - ox);
-  bool any = false;
+  bool any[2] = {false, false};
   for (int blk = 0; blk < 2; blk++)
     for (int cz = oz; cz < min(oz + QT, C.nc[2]); cz++)
       for (int cy = oy; cy < min(oy + QT, C.nc[1]); cy++) {
         const uint32_t key = (uint32_t)blk * C.ncells + (uint32_t)ox +
                              (uint32_t)C.nc[0] * ((uint32_t)cy + (uint32_t)C.nc[1] * (uint32_t)cz);
-        any = any || cellstart[key + w] != cellstart[key];
+        any[blk] = any[blk] || cellstart[key + w] != cellstart[key];
       }
-  if (any) ws[4 + atomicAdd(&ws[0], 1u)] = (uint32_t)t;
+  // Tiles with fluid centre particles fill the list from the front, tiles with boundary particles only (short ones:
+  // B <- F pairs, no momentum) from the back: the CTAs take the list in order, so the launch ends with short tiles
+  // (4.720 against 4.787 ms per pass on config 2).
+  if (any[1]) ws[4 + atomicAdd(&ws[0], 1u)] = (uint32_t)t;
+  else if (any[0]) ws[4 + (uint32_t)ntiles - 1u - atomicAdd(&ws[2], 1u)] = (uint32_t)t;
 }
 
 // Persistent kernel: one CTA per SM takes active tiles from the list until it is used up.
@@ -629,7 +634,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   }
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t n_active = A.tile_ws[0];
+  const uint32_t n_front = A.tile_ws[0], n_active = n_front + A.tile_ws[2];   // fluid tiles from the front, boundary-only ones from the back
+  const uint32_t n_tiles_all = (uint32_t)(ntx * nty) * (uint32_t)((C.nc[2] + QT - 1) / QT);
   float f2max = 0.f, viscmax = 0.f;   // f2max: overflow path only (k_quad_fmax covers every fluid particle)
   unsigned int nbsum = 0;
 
@@ -638,7 +644,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   if (tid == 0) s_tile = atomicAdd(&A.tile_ws[1], 1u);
   __syncthreads();
   if (s_tile >= n_active) break;
-  const int tile = (int)A.tile_ws[4 + s_tile];
+  const int tile = (int)A.tile_ws[4 + (s_tile < n_front ? s_tile : n_tiles_all - 1u - (s_tile - n_front))];
   const int tx = tile % ntx, ty = (tile / ntx) % nty, tz = tile / (ntx * nty);
   const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
 
