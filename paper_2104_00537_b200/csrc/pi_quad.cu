@@ -1,28 +1,30 @@
 // Particle interaction (PI) task, "quad" kernel for sm_100a: 3-D, cells of size 2h (cell_div = 1).
 //
-// A persistent CTA (one per SM) takes 2x2x2-cell tiles from a device-built list of non-empty tiles and stages each
-// tile plus a one-cell halo in shared memory with exact tile-centred coordinates (C1/C2 hold bit for bit).  The
-// work of a warp is organised so that every shared-memory access of the hot loops is bank-conflict free and the
-// pair arithmetic runs on packed FP32x2 instructions (FFMA2/FADD2/FMUL2, new on sm_100):
+// A persistent CTA (one per SM) takes 2x2x2-cell tiles from a device-built list of non-empty tiles (tiles with fluid
+// first, boundary-only tiles last) and stages each tile plus a one-cell halo in shared memory with TMA bulk copies
+// (every cell is one contiguous range of the sorted arrays, C3); an in-place pass rewrites the positions as exact
+// tile-centred coordinates (C1/C2 hold bit for bit) and builds a half-precision test record per particle.
 //
-//   a-group : 8 particles a of one cell = 4 quarter-warps x 2.  Quarter-warp q owns the pair (a_2q, a_2q+1);
-//             its 8 lanes r = 0..7 own the candidates b whose staged index is congruent to r modulo 8.
-//   T phase : (test) lane (q, r) walks the candidate rows 16 candidates per step: one LDS.128 brings the
-//             half-precision test records of candidates 16g+r and 16g+r+8 (packed as half2), three HFMA2 and
-//             one HSET2 per a evaluate the expanded-form prefilter |b|^2 - 2 a.b < R^2 + margin - |a|^2 for
-//             both candidates at once.  The prefilter is conservative (margin > its rounding error, DESIGN.md
-//             5.2); the bits of both a are OR-ed into one 32-bit word per 16 steps; non-empty words go to the
-//             lane's private word list in shared memory (no votes, no compaction across lanes).
-//   P phase : (pair) every lane pops the set bits of its own words (one FLO per pop).  Lane r only ever holds
-//             candidates of residue r, so the 8 records loaded by a quarter-warp in one step lie in 8 different
-//             bank groups (two conflict-free LDS.128 per popped b).  The trip count is the warp maximum of the
-//             per-lane pop counts (one REDUX per round), so the loop carries no vote.  Every popped b is
-//             evaluated against BOTH a of the lane with packed FP32x2 arithmetic, b entering as a broadcast
-//             scalar operand.  The exact
+//   work unit : 16 particles a of one centre cell x half of the 27-cell stencil (part 0 / part 1: disjoint row sets with
+//             about equal numbers of neighbours); the two units of a group add their partial sums into the zeroed
+//             output with atomics.  Units are handed out dynamically to the 16 warps.
+//   lanes   : lane (g, t) = (lane / 4, lane % 4).  The four lanes of g own the pair (a_g, a_g+8) of the group; lane t
+//             owns the candidates b whose staged index is congruent to 2t or 2t + 1 modulo 8.
+//   T phase : (test) one mma.sync m16n8k8 (f16) per 8 candidates evaluates the expanded-form prefilter
+//             D = |a|^2 - 2 a.b + |b|^2 - (R^2 + margin) for the 16 a of the warp (-2a split into two halves for
+//             precision); b is a candidate of a iff D < 0.  The prefilter is conservative (margin > its rounding
+//             error).  The sign bits of both a of a lane are OR-ed and collected, QB steps at a time,
+//             into one 32-bit word per residue stream and 32 steps; non-empty words go to the lane's private word
+//             list in shared memory together with the address of the record of bit 0 (no votes, no compaction).
+//   P phase : (pair) every lane pops the set bits of its own words (one FLO per pop) and loads the two records of b
+//             (LDS.128 each).  The trip count is the warp maximum of the per-lane pop counts (one REDUX per round),
+//             so the loop carries no vote; a lane out of bits evaluates a dummy record far away.  Every popped b is
+//             evaluated against BOTH a of the lane with packed FP32x2 arithmetic (FFMA2/FADD2/FMUL2, new on sm_100),
+//             b entering as a broadcast scalar operand; the sums are packed in-place FFMA2 as well.  The exact
 //             canonical predicate C2 (fp32, individually rounded) decides membership; a b that is a neighbour
 //             of only one of the two a contributes exactly 0 to the other (the kernel weight is clamped at 0).
-//   reduce  : the partial sums of the 8 lanes of a quarter-warp are combined with 3 butterfly shuffles
-//             (fixed order, deterministic) and lane r = 0 writes the two results.
+//   reduce  : the partial sums of the 4 lanes of a pair are combined with 2 butterfly shuffles (fixed order) and
+//             lane t = 0 adds the two results to the output.
 //
 // What is kept from the paper: cell-linked list, particles sorted by cell, fp32 cell-relative positions
 // (PAPER.md:558, 572).  What differs: the thread-per-particle loop with a branch per candidate.
