@@ -498,7 +498,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
     Q_LOAD(addr, pbA, vbA)                                                                             \
     Q_POP(addr)                                                                                        \
     Q_UNPACK()                                                                                         \
-    _Pragma("unroll 1")                                                                                \
+    _Pragma("unroll 2") /* two trips = four steps per iteration: 4.675 against 4.722 ms (unroll 3: 4.760, 4: 4.819) */     \
     for (unsigned k = 0; k < nmax; k += 2) { /* at most one surplus evaluation of dummy records */     \
       Q_PACK()                                                                                         \
       Q_LOAD(addr, pbB, vbB)   /* record of step k + 1: its address was popped during step k - 1 */    \
