@@ -641,12 +641,16 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   float f2max = 0.f, viscmax = 0.f;   // f2max: overflow path only (k_quad_fmax covers every fluid particle)
   unsigned int nbsum = 0;
 
+ // One thread claims the next tile while the CTA computes the current one (the atomic is a global round trip that
+ // would otherwise stall all 16 warps once per tile); the result is read after the next tile barrier
+ // (4.658 against 4.676 ms; reading the tile id ahead as well is slower: 4.677).
+ if (tid == 0) s_tile = atomicAdd(&A.tile_ws[1], 1u);
  for (;;) {
   __syncthreads();                                  // every warp is done with the previous tile's shared memory
-  if (tid == 0) s_tile = atomicAdd(&A.tile_ws[1], 1u);
-  __syncthreads();
-  if (s_tile >= n_active) break;
-  const int tile = (int)A.tile_ws[4 + (s_tile < n_front ? s_tile : n_tiles_all - 1u - (s_tile - n_front))];
+  const uint32_t cur_tile = s_tile;
+  if (cur_tile >= n_active) break;
+  bool claimed = false;
+  const int tile = (int)A.tile_ws[4 + (cur_tile < n_front ? cur_tile : n_tiles_all - 1u - (cur_tile - n_front))];
   const int tx = tile % ntx, ty = (tile / ntx) % nty, tz = tile / (ntx * nty);
   const int ox = tx * QT, oy = ty * QT, oz = tz * QT;
 
@@ -785,6 +789,10 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   }
   __syncthreads();
 
+  if (!claimed) {                                   // every thread has read s_tile (two barriers ago)
+    if (tid == NT - 1) s_tile = atomicAdd(&A.tile_ws[1], 1u);
+    claimed = true;
+  }
   // 4. a-groups, taken dynamically by the warps
   uint2* bmw = S.bm + warp * QSLOT * 32;
   while (true) {
@@ -804,6 +812,7 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   }
   if (part == 0) break;
   }   // parts
+  if (!claimed && tid == NT - 1) s_tile = atomicAdd(&A.tile_ws[1], 1u);   // no (half) tile reached the a-groups
  }   // tiles
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
