@@ -211,6 +211,42 @@ int sph_get_info(sph_ctx* ctx, sph_info* info);
 int sph_set_profiling(sph_ctx* ctx, int32_t on);
 int sph_get_timings(sph_ctx* ctx, sph_timings* out);
 
+/* The neighbour-list sort ("the particles ... are sorted according to the cell to which they belong";
+ * order convention C3) on its own, for callers that are not allowed to allocate device memory.
+ *
+ * Who that is: a host code that took all of the GPU's memory into its own pool at start-up, so that a cudaMalloc made
+ * behind its back fails or eats into what it thinks it has (a coupled solver with a fixed memory budget, a plug-in that
+ * gets no allocator callback to put into sph_params.dev_alloc); and a caller inside a time loop that must not stall,
+ * because cudaMalloc and cudaFree make every stream of the device wait.  The context calls above take their sort work
+ * space from dev_alloc / cudaMalloc in sph_load_particles.  This call does not: it never calls cudaMalloc, cudaFree or
+ * any routine that allocates.  Its work space (ping-pong buffers, digit histograms) is a fixed array compiled into the
+ * library, about 8.3 MiB, which each GPU that loads the library keeps until the process ends.  The price is a size
+ * limit: n <= SPH_SORT_STATIC_MAX_N.
+ *
+ *   key         device, uint32[n]: one key per particle, e.g. the C3 cell key; only read.
+ *   n           number of keys; 0 is a no-op; n > SPH_SORT_STATIC_MAX_N returns SPH_E_OVERFLOW and does nothing.
+ *   key_bits    the keys are ordered by their low key_bits bits (1..32; 8 bits per pass), so any higher bit should be 0.
+ *   key_sorted  device, uint32[n], written: the keys in ascending order.
+ *   perm        device, uint32[n], written: perm[j] = position in `key` of the j-th sorted key.  Equal keys keep their
+ *               input order (stable), so the result is unique and equals SPH_KEY / SPH_PERM of the context path.
+ *   cuda_stream cudaStream_t (NULL = legacy default stream) of the CURRENT device; the three arrays live on that device,
+ *               are owned by the caller and must not overlap.  The work is only enqueued; the call does not wait for it.
+ *   errmsg      NULL, or host memory of errmsg_bytes bytes that receives a message when the result is not SPH_OK.
+ *
+ * Returns SPH_OK, SPH_E_BADARG (negative n, key_bits out of range, NULL or aliased arrays), SPH_E_OVERFLOW (n above
+ * the limit) or SPH_E_CUDA.
+ *
+ * First call on a device: the library looks up where its work space lives on that device (cudaGetSymbolAddress) and
+ * remembers it; the device must be current on the calling thread.  Make this first call during set-up, before any
+ * stream capture is begun.
+ * Sharing: all calls on one device use the same work space, and it keeps whatever the previous call left (the call
+ * clears the part that has to start at zero itself).  Two calls whose GPU work can overlap in time -- different streams
+ * without an ordering between them, or two host threads -- race on it and give wrong results; put them on one stream or
+ * order them with events. */
+#define SPH_SORT_STATIC_MAX_N 1048576
+int sph_sort_keys_static(const uint32_t* key, int64_t n, int32_t key_bits, uint32_t* key_sorted, uint32_t* perm,
+                         void* cuda_stream, char* errmsg, size_t errmsg_bytes);
+
 /* Message of the last error on this context ("" if none).  Valid until the next call.
  * With ctx = NULL: the reason of the last failed sph_create on the calling thread. */
 const char* sph_last_error(const sph_ctx* ctx);

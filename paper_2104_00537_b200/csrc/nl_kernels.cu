@@ -4,6 +4,11 @@
 // their data are sorted according to the cell to which they belong and an index array with the first
 // and last particle of each cell is created."  Canonical key / order / range conventions: C3.
 // All of this is integer work and must be bit-exact against the oracle.
+#include <stdarg.h>
+#include <stdio.h>
+
+#include <mutex>
+
 #include "sph_internal.cuh"
 
 namespace {
@@ -226,4 +231,125 @@ void nl_reorder(const DevConsts& C, const ParticleSet& src, const ParticleSet& d
                 int64_t n, bool with_n_state, cudaStream_t s) {
   if (n == 0) return;
   k_reorder<<<grid_for(n, 256), 256, 0, s>>>(C, src, dst, idx, n, with_n_state ? 1 : 0);
+}
+
+// =====================================================================================================================
+// sph_sort_keys_static (include/sph.h): the a2 radix sort above for callers that must not allocate.
+//
+// The context path (build_nl in sph_api.cu) gets its sort work space -- the ping-pong (key, index) buffers, the
+// per-block digit histograms and the digit totals -- from sph_params.dev_alloc or cudaMalloc at sph_load_particles.
+// A host program that has already handed every byte of HBM to its own pool, or that calls the sort from inside a
+// solver loop it cannot afford to stall (cudaMalloc and cudaFree synchronise the whole device), has neither option.
+// For those callers the same three kernels run here on a work space that is part of the library image: one
+// file-scope __device__ array, sized for SPH_SORT_STATIC_MAX_N pairs, which every GPU that loads the library holds
+// until the process exits (about 8.3 MiB).
+//
+// Note for whoever edits this: in HOST code the name g_sort_scratch is only a handle of the symbol.  It is not a device
+// address and must never be given to a kernel or to cudaMemsetAsync; the address on the current device comes from
+// cudaGetSymbolAddress, once per device (sort_scratch_on_current_device).
+// =====================================================================================================================
+namespace {
+
+constexpr int64_t ST_MAX_N = SPH_SORT_STATIC_MAX_N;
+constexpr size_t ST_MAX_BLOCKS = (size_t)((ST_MAX_N + RS_TILE - 1) / RS_TILE);
+// layout, in 32-bit words (every part starts on a 256-byte boundary):
+constexpr size_t ST_OFF_KEY = 0;                                        // ping-pong keys            [ST_MAX_N]
+constexpr size_t ST_OFF_IDX = ST_OFF_KEY + (size_t)ST_MAX_N;            // ping-pong indices         [ST_MAX_N]
+constexpr size_t ST_OFF_HIST = ST_OFF_IDX + (size_t)ST_MAX_N;           // per-block digit histogram [256][nblocks]
+constexpr size_t ST_OFF_TOTAL = ST_OFF_HIST + ST_MAX_BLOCKS * RS_RADIX; // digit totals, 4 passes    [4][256]
+constexpr size_t ST_WORDS = ST_OFF_TOTAL + 4 * RS_RADIX;
+static_assert(ST_MAX_N % 64 == 0 && (ST_MAX_BLOCKS * RS_RADIX) % 64 == 0, "parts of the work space are 256-byte aligned");
+
+static __device__ __align__(256) uint32_t g_sort_scratch[ST_WORDS];
+
+constexpr int ST_MAX_DEVICES = 64;
+uint32_t* g_scratch_addr[ST_MAX_DEVICES];   // device address of g_sort_scratch, per device ordinal; 0 = not looked up yet
+std::mutex g_scratch_mu;
+
+// Address of the work space on the device that is current on the calling thread.  The first call on a device asks the
+// runtime for it (this also makes the runtime load the module there); later calls read the cached pointer.
+cudaError_t sort_scratch_on_current_device(uint32_t** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= ST_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_scratch_mu);
+  if (!g_scratch_addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_sort_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_scratch_addr[dev] = (uint32_t*)p;
+  }
+  *out = g_scratch_addr[dev];
+  return cudaSuccess;
+}
+
+int static_sort_fail(int code, char* errmsg, size_t errmsg_bytes, const char* fmt, ...) {
+  if (errmsg && errmsg_bytes) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(errmsg, errmsg_bytes, fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+}  // namespace
+
+extern "C" __attribute__((visibility("default"))) int sph_sort_keys_static(const uint32_t* key, int64_t n,
+                                                                           int32_t key_bits, uint32_t* key_sorted,
+                                                                           uint32_t* perm, void* cuda_stream,
+                                                                           char* errmsg, size_t errmsg_bytes) {
+  if (errmsg && errmsg_bytes) errmsg[0] = 0;
+  if (n < 0) return static_sort_fail(SPH_E_BADARG, errmsg, errmsg_bytes, "sph_sort_keys_static: n = %lld is negative", (long long)n);
+  if (key_bits < 1 || key_bits > 32)
+    return static_sort_fail(SPH_E_BADARG, errmsg, errmsg_bytes, "sph_sort_keys_static: key_bits = %d, must be 1..32", (int)key_bits);
+  if (n > ST_MAX_N)
+    return static_sort_fail(SPH_E_OVERFLOW, errmsg, errmsg_bytes,
+                            "sph_sort_keys_static: n = %lld exceeds SPH_SORT_STATIC_MAX_N = %lld, the size the built-in work "
+                            "space was compiled for; larger sorts need a context (sph_create), which allocates",
+                            (long long)n, (long long)ST_MAX_N);
+  if (n == 0) return SPH_OK;
+  if (!key || !key_sorted || !perm)
+    return static_sort_fail(SPH_E_BADARG, errmsg, errmsg_bytes, "sph_sort_keys_static: null key, key_sorted or perm pointer");
+  if (key == key_sorted || key == perm || key_sorted == perm)
+    return static_sort_fail(SPH_E_BADARG, errmsg, errmsg_bytes, "sph_sort_keys_static: key, key_sorted and perm must be three different arrays");
+
+  uint32_t* ws = nullptr;
+  cudaError_t e = sort_scratch_on_current_device(&ws);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return static_sort_fail(SPH_E_CUDA, errmsg, errmsg_bytes, "sph_sort_keys_static: cudaGetSymbolAddress(work space): %s",
+                            cudaGetErrorString(e));
+  }
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  uint32_t* tmp_key = ws + ST_OFF_KEY;
+  uint32_t* tmp_idx = ws + ST_OFF_IDX;
+  uint32_t* block_hist = ws + ST_OFF_HIST;
+  uint32_t* digit_total = ws + ST_OFF_TOTAL;
+
+  const uint32_t nblocks = (uint32_t)((n + RS_TILE - 1) / RS_TILE);
+  const int passes = (key_bits + 7) / 8;
+  // The work space still holds what the previous call left.  Only the digit totals are accumulated into (atomicAdd in
+  // k_rs_hist) and have to start at zero; the histograms and the ping-pong buffers are fully written before being read.
+  e = cudaMemsetAsync(digit_total, 0, sizeof(uint32_t) * RS_RADIX * 4, s);
+  // Pass p writes to the caller's arrays when an even number of passes follow it, else to the work space, so the last
+  // pass always lands in (key_sorted, perm) and the caller's input is only ever read.
+  const uint32_t *kin = key, *iin = nullptr;
+  for (int p = 0; p < passes && e == cudaSuccess; p++) {
+    const bool to_caller = ((passes - 1 - p) & 1) == 0;
+    uint32_t* kout = to_caller ? key_sorted : tmp_key;
+    uint32_t* iout = to_caller ? perm : tmp_idx;
+    const int shift = 8 * p;
+    k_rs_hist<<<nblocks, RS_THREADS, 0, s>>>(kin, n, shift, nblocks, block_hist, digit_total + p * RS_RADIX);
+    k_rs_scan<<<RS_RADIX, RS_THREADS, 0, s>>>(block_hist, nblocks, digit_total + p * RS_RADIX);
+    k_rs_scatter<<<nblocks, RS_THREADS, 0, s>>>(kin, iin, n, shift, nblocks, block_hist, kout, iout, p == 0);
+    kin = kout;
+    iin = iout;
+    e = cudaGetLastError();
+  }
+  if (e != cudaSuccess)
+    return static_sort_fail(SPH_E_CUDA, errmsg, errmsg_bytes, "sph_sort_keys_static: %s", cudaGetErrorString(e));
+  return SPH_OK;
 }

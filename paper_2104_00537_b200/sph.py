@@ -86,7 +86,8 @@ class SphTimings(C.Structure):
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_load_particles", "sph_set_motion", "sph_set_boundary_normals",
            "sph_compute_interactions", "sph_step", "sph_read_state", "sph_read_fields", "sph_get_info",
-           "sph_set_profiling", "sph_get_timings", "sph_last_error", "sph_version"]
+           "sph_set_profiling", "sph_get_timings", "sph_last_error", "sph_version", "sph_sort_keys_static"]
+SPH_SORT_STATIC_MAX_N = 1 << 20
 
 
 def _load():
@@ -112,6 +113,7 @@ def _load():
     L.sph_last_error.argtypes = [vp]
     L.sph_last_error.restype = C.c_char_p
     L.sph_version.restype = C.c_char_p
+    L.sph_sort_keys_static.argtypes = [vp, C.c_int64, C.c_int32, vp, vp, vp, C.c_char_p, C.c_size_t]
     for name in EXPORTS:
         if name not in ("sph_destroy", "sph_last_error", "sph_version"):
             getattr(L, name).restype = C.c_int
@@ -129,6 +131,19 @@ class SphError(RuntimeError):
 
 def version() -> str:
     return lib.sph_version().decode()
+
+
+def sort_keys_static(key_ptr, n, key_bits, key_sorted_ptr, perm_ptr, stream_ptr=None):
+    """sph_sort_keys_static: the neighbour-list sort for callers that may not allocate device memory (a host code that
+    owns all of HBM through its own pool, or a loop that cannot take the device-wide stall of cudaMalloc / cudaFree).
+    The work space is a fixed array inside the library, so n <= SPH_SORT_STATIC_MAX_N.  All three pointers are raw
+    DEVICE addresses of uint32[n] arrays on the current device (e.g. tensor.data_ptr()); stream_ptr is a cudaStream_t
+    value (None = legacy default stream).  Only enqueues work.  The first call on a device does a one-off address look-up
+    and belongs in set-up code; calls that can overlap on the GPU share the work space and race (see include/sph.h)."""
+    msg = C.create_string_buffer(512)
+    rc = lib.sph_sort_keys_static(key_ptr, n, key_bits, key_sorted_ptr, perm_ptr, stream_ptr, msg, len(msg))
+    if rc != SPH_OK:
+        raise SphError(rc, msg.value.decode())
 
 
 class Sph:
