@@ -748,7 +748,9 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   // 2. stage the particles: the sorted arrays hold every cell as one contiguous range (C3), so each non-empty staged
   //    range is two TMA bulk copies (positions + density, velocities + pressure) straight into shared memory,
   //    completing on one mbarrier (no register staging, all copies of the tile in flight at once).
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic-proxy accesses of this memory come first
+  //    (The generic-proxy accesses of the previous tile were fenced by the threads that made them, before the barrier,
+  //    at the end of step 4; this second fence in the issuing threads is kept as well: one instruction per tile.)
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   if (tid == 0) mbar_arrive_expect_tx(mbar_s, total * 32u);
   for (int rr = tid; rr < QNR; rr += NT) {
     const uint32_t n = s_cnt[rr];
@@ -810,6 +812,10 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     if (blk == 1) process_group<true, LAM, FOURT>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
     else process_group<false, false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
   }
+  // This thread is done with the staged records: its generic-proxy accesses (the in-place rewrite of step 3, the dummy
+  // record, the reads of step 4) are ordered before the next barrier here, in the thread that made them, so that the
+  // bulk copies (async proxy) of the next tile or half tile, issued after that barrier, may overwrite the memory.
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   if (part == 0) break;
   }   // parts
   if (!claimed && tid == NT - 1) s_tile = atomicAdd(&A.tile_ws[1], 1u);   // no (half) tile reached the a-groups
