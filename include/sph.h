@@ -142,8 +142,10 @@ enum sph_field {
   SPH_CELL = 10,      /* int32[n*3]   canonical cell coordinates (C1)                               */
   SPH_OFFSET = 11,    /* float[n*3]   canonical in-cell offsets u in [0,1) on the 2^-22 grid (C1)   */
   SPH_PRESS = 12,     /* float[n]     P of the last reorder (Eq. 28)                                */
-  SPH_CONC = 13,      /* float[n]     particle concentration C_a of the last pass (Eq. 53; shift_model = 1) */
-  SPH_SHIFT = 14      /* float[n*3]   shifting velocity delta r_a / dt of the last pass (Eq. 40-41, 54); 0 for boundary */
+  SPH_CONC = 13,      /* float[n]     particle concentration C_a of the last pass (Eq. 53; shift_model = 1);    */
+                      /*              0 for particles out of the grid (A16)                                     */
+  SPH_SHIFT = 14      /* float[n*3]   shifting velocity delta r_a / dt of the last pass (Eq. 40-41, 54); 0 for  */
+                      /*              boundary particles and for particles out of the grid                      */
 };
 
 /* Create a context.  Validates params, derives constants (m, B, alpha_D, eta^2, cell grid).

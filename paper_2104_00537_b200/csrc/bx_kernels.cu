@@ -233,10 +233,14 @@ __device__ __forceinline__ void for_each_neighbour(const DevConsts& C, const flo
 // C_a = V_a W(0) + sum_b V_b W_ab   (Eq. 53, A27); W = alpha_D (1 - q/2)^4 (2q + 1) (Eq. 11)
 template <int DIM>
 __global__ void __launch_bounds__(128) k_conc(DevConsts C, const float4* __restrict__ posu, const int* __restrict__ cell,
-                                              const uint32_t* __restrict__ cellstart, double* __restrict__ conc) {
+                                              const uint32_t* __restrict__ cellstart, double* __restrict__ conc,
+                                              uint32_t n) {
   const uint32_t n_active = cellstart[2u * C.ncells];
   const uint32_t a = blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= n_active) return;
+  if (a >= n_active) {                        // particles out of the grid (sorted last, C3) take no part: C_a = 0
+    if (a < n) conc[a] = 0.0;
+    return;
+  }
   const float4 pa = posu[a];
   double sum = (double)(fast_rcp(pa.w));      // self term: w = 1, q = 0
   for_each_neighbour<DIM>(C, posu, cellstart, a, pa, cell[a],
@@ -252,11 +256,13 @@ template <int DIM>
 __global__ void __launch_bounds__(128) k_shift(DevConsts C, const float4* __restrict__ posu,
                                                const float4* __restrict__ velp, const int* __restrict__ cell,
                                                const uint32_t* __restrict__ cellstart, const double* __restrict__ conc,
-                                               float4* __restrict__ shiftv) {
+                                               float4* __restrict__ shiftv, uint32_t n) {
   const uint32_t n_bound = cellstart[C.ncells], n_active = cellstart[2u * C.ncells];
   const uint32_t a = blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= n_active) return;
-  if (a < n_bound) { shiftv[a] = make_float4(0.f, 0.f, 0.f, 0.f); return; }
+  if (a >= n) return;
+  // boundary particles and particles out of the grid are not shifted; the slot of an out-of-grid particle would
+  // otherwise keep the vector some other particle left there on an earlier pass
+  if (a < n_bound || a >= n_active) { shiftv[a] = make_float4(0.f, 0.f, 0.f, 0.f); return; }
   const float4 pa = posu[a];
   const double Ca = conc[a];
   float gx = 0.f, gy = 0.f, gz = 0.f;
@@ -298,10 +304,10 @@ void bx_shift(const DevConsts& C, const ParticleSet& P, const uint32_t* cellstar
   if (n == 0) return;
   const unsigned grid = (unsigned)((n + 127) / 128);
   if (C.dim == 3) {
-    k_conc<3><<<grid, 128, 0, s>>>(C, P.posu, P.cell, cellstart, conc);
-    k_shift<3><<<grid, 128, 0, s>>>(C, P.posu, P.velp, P.cell, cellstart, conc, shiftv);
+    k_conc<3><<<grid, 128, 0, s>>>(C, P.posu, P.cell, cellstart, conc, (uint32_t)n);
+    k_shift<3><<<grid, 128, 0, s>>>(C, P.posu, P.velp, P.cell, cellstart, conc, shiftv, (uint32_t)n);
   } else {
-    k_conc<2><<<grid, 128, 0, s>>>(C, P.posu, P.cell, cellstart, conc);
-    k_shift<2><<<grid, 128, 0, s>>>(C, P.posu, P.velp, P.cell, cellstart, conc, shiftv);
+    k_conc<2><<<grid, 128, 0, s>>>(C, P.posu, P.cell, cellstart, conc, (uint32_t)n);
+    k_shift<2><<<grid, 128, 0, s>>>(C, P.posu, P.velp, P.cell, cellstart, conc, shiftv, (uint32_t)n);
   }
 }

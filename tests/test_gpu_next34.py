@@ -212,6 +212,33 @@ def test_shift_random_clouds(sph, dim, periodic, cell_div):
     check_shift_one_pass(sph, c, 0)
 
 
+def test_shift_fields_are_zero_for_particles_out_of_the_grid(sph):
+    """include/sph.h: SPH_CONC and SPH_SHIFT are 0 for particles out of the grid (A16), as in the oracle, which skips
+    them.  The first pass fills every sorted slot; after the reload three fluid particles have left the grid, and their
+    slots (sorted last, C3) must not keep what other particles left there."""
+    c = perturbed(wl.config(0), 45, vel_sigma=0.3)
+    p = dict(c.params, shift_model=1, shift_coef=2.0)
+    esc = np.flatnonzero(c.ptype == 0)[[5, 600, 4000]]
+    pos2 = c.pos.copy()
+    pos2[esc, 2] += 50.0
+    st = oracle.State(p, pos2, c.vel, c.rho, c.ptype)
+    assert st.out.sum() == 3 and (st.out[esc] == 1).all()
+    conc = oracle.concentration(p, st.cell, st.u, st.out, st.rho, st.ptype)
+    shift, _ = oracle.shift_velocity(p, st.cell, st.u, st.out, st.vel, st.rho, st.ptype, conc)
+    assert (conc[esc] == 0).all() and (shift[esc] == 0).all()
+    with sph.Sph(p) as S:
+        S.load_case(c)
+        S.compute_interactions()
+        assert (S.read_state(sph.SPH_CONC) > 0).all()
+        S.load_particles(pos2, c.vel, c.rho, c.ptype)
+        S.compute_interactions()
+        assert S.get_info().n_out == 3
+        got_c, got_s = S.read_state(sph.SPH_CONC), S.read_state(sph.SPH_SHIFT)
+        assert (got_c[esc] == 0).all() and (got_s[esc] == 0).all()
+        assert_close("C", got_c, conc, rtol=1e-6, floor=0)          # every particle, the escaped ones included
+        assert_close("shift", got_s, shift)
+
+
 @pytest.mark.parametrize("pi_kernel", KERNELS)
 @pytest.mark.parametrize("integrator", [0, 1])
 def test_shift_ten_steps(sph, pi_kernel, integrator):
