@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(128) k_shift(DevConsts C, const float4* __rest
   const float4 va = velp[a];
   const float ds = C.shift_ds * sqrtf(fmaf(va.z, va.z, fmaf(va.y, va.y, va.x * va.x)));   // D_s / dt (Eq. 41)
   float4 out;
-  if ((float)Ca < C.shift_fs_conc) {              // Eq. 54 with n = -grad C / |grad C| (A29)
+  if (Ca < C.shift_fs_conc) {                     // Eq. 54 with n = -grad C / |grad C| (A29); a discontinuous switch, so in double
     const float gn = sqrtf(fmaf(gz, gz, fmaf(gy, gy, gx * gx)));
     const float fac = gn > 0.f ? -ds * C.shift_alpha_n * (-gn - C.shift_beta_n) / gn : 0.f;
     out = make_float4(-fac * gx, -fac * gy, -fac * gz, 0.f);

@@ -270,7 +270,7 @@ int derive(const sph_params* p, DevConsts& C, std::string& why) {
   C.c_w = (float)(m * aD);
   C.c_gw = (float)(m * Cf * cs);
   C.shift_ds = (float)((p->shift_coef > 0.0 ? p->shift_coef : 2.0) * p->h);
-  C.shift_fs_conc = (float)p->shift_fs_conc;
+  C.shift_fs_conc = p->shift_fs_conc;
   C.shift_alpha_n = (float)p->shift_alpha_n;
   C.shift_beta_n = (float)p->shift_beta_n;
   return SPH_OK;

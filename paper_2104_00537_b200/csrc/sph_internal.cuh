@@ -42,7 +42,8 @@ struct DevConsts {
   float c_w;               // m alpha_D          : V_b W_ab = c_w (1/rho_b) w^4 (2q + 1)
   float c_gw;              // m Cf cs            : V_b grad_a W_ab = c_gw (1/rho_b) w^3 du
   float shift_ds;          // A_s h              : D_s / dt = shift_ds |v_a|   (Eq. 41)
-  float shift_fs_conc, shift_alpha_n, shift_beta_n;
+  float shift_alpha_n, shift_beta_n;
+  double shift_fs_conc;    // free-surface switch of Eq. 54: compared with the double C_a, as the oracle does
 };
 
 // Tait EOS, Eq. 28, evaluated without the cancellation of (rho/rho0)^gamma - 1:
