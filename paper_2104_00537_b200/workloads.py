@@ -170,10 +170,15 @@ def dam_break(name, dim, dp, tank_sites, fluid_sites, jitter, seed, c0_height,
     dmax = (nx * dp + m, (ny * dp + m) if dim == 3 else 0.0, top_factor * nz * dp)
     p = _params(dim, dp, 1.2, c0, g, dmin, dmax, cell_div=cell_div)
     lo, hi = (0.0, 0.0, 0.0), (nx * dp, ny * dp, nz * dp)
+    normals = box_normals(pos, ptype, lo, hi, dim=dim)
+    if obstacle is not None:
+        (i0, j0, k0), (ni, nj, nk) = obstacle
+        normals += obstacle_normals(pos, ptype, (i0 * dp, j0 * dp, k0 * dp),
+                                    ((i0 + ni) * dp, (j0 + nj) * dp, (k0 + nk) * dp), lo, hi, dim=dim)
     return Case(name, np.ascontiguousarray(pos), vel, rho, ptype, p, nsteps=nsteps,
                 notes=f"dam break dim={dim} dp={dp} tank={tank_sites} fluid={fluid_sites} "
                       f"jitter={jitter} seed={seed}",
-                normals=box_normals(pos, ptype, lo, hi, dim=dim), box=(lo, hi))
+                normals=normals, box=(lo, hi))
 
 
 def box_normals(pos, ptype, lo, hi, dim=3, open_top=True):
@@ -192,6 +197,31 @@ def box_normals(pos, ptype, lo, hi, dim=3, open_top=True):
         if not (ax == 2 and open_top):
             nrm[above, ax] = hi[ax] - x[above]
     nrm[np.asarray(ptype) == FLUID] = 0.0
+    return nrm
+
+
+def obstacle_normals(pos, ptype, o_lo, o_hi, lo, hi, dim=3):
+    """mDBC input for a solid box obstacle [o_lo, o_hi] standing inside the tank [lo, hi]: for every boundary particle
+    inside the obstacle, the vector to the nearest obstacle face that is wetted, i.e. not lying on a tank plane (the
+    faces are the interface: half a spacing outside the outermost particle layer).  A tie between faces goes to the
+    lower axis, then to the lower side.  Pure geometry; all other rows are 0, so the result adds to box_normals."""
+    pos = np.asarray(pos, np.float64)
+    nrm = np.zeros_like(pos)
+    axes = [ax for ax in range(3) if not (dim == 2 and ax == 1)]
+    inside = np.asarray(ptype) != FLUID
+    for ax in axes:
+        inside &= (pos[:, ax] > o_lo[ax]) & (pos[:, ax] < o_hi[ax])
+    rows = np.flatnonzero(inside)
+    best = np.full(rows.size, np.inf)
+    for ax in axes:
+        for face, wetted in ((o_lo[ax], o_lo[ax] > lo[ax]), (o_hi[ax], o_hi[ax] < hi[ax])):
+            if not wetted:
+                continue
+            d = face - pos[rows, ax]
+            closer = np.abs(d) < best
+            best[closer] = np.abs(d[closer])
+            nrm[rows[closer]] = 0.0
+            nrm[rows[closer], ax] = d[closer]
     return nrm
 
 

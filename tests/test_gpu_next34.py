@@ -103,6 +103,17 @@ def test_mdbc_2d_and_cell_div(sph, cell_div):
     check_mdbc_one_pass(sph, perturbed(c, 34), 1, 1)
 
 
+@pytest.mark.parametrize("slip", [0, 1])
+def test_mdbc_dam_break_with_obstacle(sph, slip):
+    """The obstacle's particles carry interface vectors of their own (workloads.obstacle_normals), so their ghost nodes
+    lie in the fluid around the obstacle: full solves must occur on the obstacle, not only on the tank."""
+    c = wl.dam_break("obstacle", 3, 0.02, (40, 20, 20), (15, 20, 15), 0.01, 4321, 0.3, obstacle=((13, 6, 0), (5, 8, 6)))
+    status = check_mdbc_one_pass(sph, perturbed(c, 37), 0, slip)
+    obs = (c.ptype != 0) & (c.pos[:, 0] > 0.26) & (c.pos[:, 0] < 0.36) & (c.pos[:, 1] > 0.12) & (c.pos[:, 1] < 0.28) & \
+          (c.pos[:, 2] > 0.0) & (c.pos[:, 2] < 0.12)
+    assert obs.sum() == 5 * 8 * 6 and (status[obs] == 1).sum() > 20
+
+
 def test_mdbc_moving_wall_no_slip(sph):
     c = with_piston(perturbed(wl.config(0), 35))
     check_mdbc_one_pass(sph, c, 3, 1)

@@ -385,3 +385,38 @@ def test_shifting_in_the_steppers_moves_positions_by_dt_times_shift(scheme):
     np.testing.assert_allclose(d, dt * s, rtol=0, atol=1.01 * q)
     np.testing.assert_array_equal(a.vel, b.vel)
     np.testing.assert_array_equal(a.rho, b.rho)
+
+
+def test_obstacle_normals_geometry():
+    """workloads.obstacle_normals (mDBC input of the obstacle dam break): every obstacle particle gets the vector to its
+    nearest wetted obstacle face -- one axis only, half a spacing for the outermost layer, never towards the floor the
+    obstacle stands on -- so that its ghost node r + 2n is its mirror image outside the obstacle; the tank's own
+    particles keep the box_normals vectors."""
+    dp = 0.02
+    obs = ((15, 6, 0), (5, 8, 6))
+    c = wl.dam_break("obstacle", 3, dp, (40, 20, 20), (15, 20, 15), 0.01, 4321, 0.3, obstacle=obs)
+    base = wl.dam_break("plain", 3, dp, (40, 20, 20), (15, 20, 15), 0.01, 4321, 0.3)
+    o_lo = np.array(obs[0]) * dp
+    o_hi = o_lo + np.array(obs[1]) * dp
+    rows = np.arange(base.n_bound, c.n_bound)                   # the obstacle's particles follow the tank's
+    assert rows.size == 5 * 8 * 6 and (c.ptype[rows] != 0).all()
+    np.testing.assert_array_equal(c.normals[:base.n_bound], base.normals[:base.n_bound])
+    assert (c.normals[c.ptype == 0] == 0).all()
+    nrm, pos = c.normals[rows], c.pos[rows]
+    assert ((nrm != 0).sum(axis=1) == 1).all()                  # one face each
+    assert (nrm[:, 2] >= 0).all()                               # the bottom face lies on the floor: not an interface
+    ghost = pos + 2.0 * nrm
+    outside = ((ghost < o_lo) | (ghost > o_hi)).any(axis=1)
+    assert outside.all()
+    # mirror image: the interface point r + n lies on an obstacle face
+    face = pos + nrm
+    on_face = (np.abs(face - o_lo) < 1e-12) | (np.abs(face - o_hi) < 1e-12)
+    assert (on_face & (nrm != 0)).any(axis=1).all()
+    # nearest face: |n| equals the smallest distance to any wetted face (all but z = 0)
+    d = np.concatenate([pos - o_lo, o_hi - pos], axis=1)[:, [0, 1, 3, 4, 5]]
+    np.testing.assert_allclose(np.abs(nrm).sum(axis=1), d.min(axis=1), rtol=0, atol=1e-15)
+    assert np.isclose(np.abs(nrm).sum(axis=1).min(), 0.5 * dp)
+    # 2-D: no y component, same rule
+    c2 = wl.dam_break("obstacle2d", 2, dp, (60, 1, 30), (20, 1, 20), 0.01, 5, 0.4, obstacle=((30, 0, 0), (4, 1, 6)))
+    ob2 = (c2.ptype != 0) & (c2.pos[:, 0] > 0.6) & (c2.pos[:, 0] < 0.68) & (c2.pos[:, 2] > 0) & (c2.pos[:, 2] < 0.12)
+    assert ob2.sum() == 24 and (c2.normals[ob2, 1] == 0).all() and ((c2.normals[ob2] != 0).sum(axis=1) == 1).all()
