@@ -161,7 +161,10 @@ void sph_destroy(sph_ctx* ctx);
  * Positions are converted on the device, in IEEE double, to the canonical state (C1):
  * s = (x-min)/cs, c = floor(s), u = rint((s-c) 2^22) 2^-22 ("relative position of the
  * particle within its cell (using single precision)").  Resets t, step count and counters.
- * This is the one host->device crossing of the run. */
+ * This is the one host->device crossing of the run.
+ * Memory: the raw inputs pass through a device staging buffer of 41 bytes per particle.  When that is at most
+ * 512 MiB (about 13 M particles) the buffer stays allocated for the next load on this context; a larger one is
+ * released before the call returns. */
 int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, const float* vel,
                        const float* rho, const uint8_t* type);
 

@@ -288,6 +288,11 @@ int alloc_set(sph_ctx* c, ParticleSet& P, int64_t n) {
   return (P.posu && P.velp && P.cell && P.id && P.type && P.posu_n && P.vel_n && P.cell_n) ? 0 : -1;
 }
 
+// sph_load_particles copies the caller's arrays into a device staging buffer (41 B per particle).  Up to this size the
+// buffer stays allocated so that a reload (a checkpoint restore, the end-to-end bench) does not allocate again; a
+// larger one (config 4: 1.4 GB) is released as soon as the load is done, so it does not lower the largest N that fits.
+constexpr size_t STAGE_KEEP_MAX_BYTES = (size_t)512 << 20;
+
 // NL task: a1 key -> a2 sort -> a3 cell ranges -> a4 reorder (+a7 EOS)
 int build_nl(sph_ctx* ctx, bool with_n_state) {
   const int64_t n = ctx->n;
@@ -551,6 +556,11 @@ SPH_EXPORT int sph_load_particles(sph_ctx* ctx, int64_t n, const double* pos, co
   ctx->n_launch += 1;
   CK(cudaGetLastError());
   CK(cudaStreamSynchronize(s));      // the caller's buffers are free again on return
+  if (ctx->stage_bytes > STAGE_KEEP_MAX_BYTES) {   // a large staging copy is not worth holding for a reload that may never come
+    dfree(ctx, ctx->stage);
+    ctx->stage = nullptr;
+    ctx->stage_bytes = 0;
+  }
   ctx->n = n;
   ctx->loaded = true;
   ctx->kstep = 0;
@@ -682,7 +692,7 @@ static size_t field_bytes(const sph_ctx* ctx, int32_t field) {
 SPH_EXPORT int sph_read_fields(sph_ctx* ctx, int32_t nfields, const int32_t* fields, void* const* dsts,
                                const size_t* dst_bytes) {
   if (!ctx || nfields < 0 || (nfields > 0 && (!fields || !dsts || !dst_bytes))) return SPH_E_BADARG;
-  if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_read_state before sph_load_particles");
+  if (!ctx->loaded) return fail(ctx, SPH_E_STATE, "sph_read_state / sph_read_fields before sph_load_particles");
   const int64_t n = ctx->n;
   cudaStream_t s = ctx->stream;
   const ParticleSet& P = ctx->set[ctx->cur];
@@ -743,7 +753,7 @@ SPH_EXPORT int sph_read_fields(sph_ctx* ctx, int32_t nfields, const int32_t* fie
   const cudaError_t e2 = cudaStreamSynchronize(s);
   if (e == cudaSuccess) e = e2;
   if (tmp) dfree(ctx, tmp);
-  if (e != cudaSuccess) return cuda_fail(ctx, e, "sph_read_state");
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "sph_read_state / sph_read_fields");
   return SPH_OK;
 }
 
