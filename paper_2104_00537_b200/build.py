@@ -3,7 +3,10 @@
 Usage: python -m paper_2104_00537_b200.build [--force]
 nvcc cross-compiles without a GPU.  Object files go to csrc/build/ (git-ignored).
 """
+import hashlib
+import json
 import os
+import socket
 import subprocess
 import sys
 from concurrent.futures import ThreadPoolExecutor
@@ -12,6 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libsph_b200.so")
+STAMP = LIB + ".stamp"     # what the library was built from, where and with which flags (git-ignored, travels with the .so)
 SOURCES = ["sph_api.cu", "nl_kernels.cu", "pi_kernels.cu", "pi_tiled.cu", "pi_quad.cu", "su_kernels.cu", "bx_kernels.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # No -use_fast_math: the canonical predicate (C2) and conversions (C1) need IEEE mul/fma/div.
@@ -26,10 +30,46 @@ def _deps():
     return d
 
 
+def source_digest() -> str:
+    """SHA-256 over the names and contents of every source the library is built from, plus the compiler flags."""
+    h = hashlib.sha256(" ".join(FLAGS).encode())
+    for p in sorted(_deps()):
+        h.update(os.path.basename(p).encode())
+        with open(p, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
+def host_id() -> str:
+    """Host name plus the kernel's boot id: two machines started from the same image share the former only."""
+    try:
+        with open("/proc/sys/kernel/random/boot_id") as f:
+            boot = f.read().strip()
+    except OSError:
+        boot = "?"
+    return f"{socket.gethostname()}/{boot}"
+
+
+def read_stamp() -> dict:
+    try:
+        with open(STAMP) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+def built_on_this_host() -> bool:
+    """True when the library in the tree was compiled on this machine from the sources as they are now."""
+    st = read_stamp()
+    return os.path.exists(LIB) and st.get("sources") == source_digest() and st.get("host") == host_id()
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile unless the library in the tree was built from exactly these sources and flags (content digest in the
+    stamp file; file times do not survive a copy of the tree to another machine)."""
     srcs = [s for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
-    newest = max(os.path.getmtime(p) for p in _deps())
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    digest = source_digest()
+    if not force and os.path.exists(LIB) and read_stamp().get("sources") == digest:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
 
@@ -50,6 +90,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.check_call([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs])
     os.replace(tmp, LIB)
+    nvcc_version = subprocess.run([NVCC, "--version"], capture_output=True, text=True).stdout.strip().splitlines()[-1:]
+    with open(STAMP, "w") as f:
+        json.dump({"sources": digest, "host": host_id(), "nvcc": " ".join(nvcc_version),
+                   "flags": FLAGS}, f, indent=1)
     return LIB
 
 
