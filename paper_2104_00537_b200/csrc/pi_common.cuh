@@ -35,6 +35,16 @@ __device__ __forceinline__ float hydrostatic_drho(const DevConsts& C, float dux,
   return C.rho0 * expm1f(log1pf(e) * C.inv_gamma);
 }
 
+// Development builds that split the fp32 error of the momentum sum of Eq. 22 into its parts (never in a release build;
+// gather kernel, pi_kernel = 1, only; reading T3, profiles/r3_momentum_error_split.md):
+//   SPH_NVCC_EXTRA=-DPI_ACC_F64   the fp32 pair terms are summed in double            -> removes the summation error
+//   SPH_NVCC_EXTRA=-DPI_TERM_F64  ... and the pair coefficient itself (r^2, 1 - q/2, (Pa + Pb) / (rho_a rho_b)) is
+//                                 evaluated in double from the stored fp32 state      -> removes the per-pair rounding;
+//                                 what is left comes from the fp32 state itself (P of the fp32 EOS, the constants)
+#if defined(PI_TERM_F64) && !defined(PI_ACC_F64)
+#define PI_ACC_F64
+#endif
+
 // Raw sums accumulated for one particle a.
 struct PairAcc {
   float sx, sy, sz;   // sum w^3 [(Pa+Pb)/(rho_a rho_b) + Pi_ab] du          -> momentum, Eq. 22
@@ -42,6 +52,9 @@ struct PairAcc {
   float sd;           // sum_F (1/rho_b) w^3 (rho_a - rho_b)                  -> density diffusion, Eq. 17-18 (A3)
   float visc;         // max |mu_ab| / c_mu
   float lx, ly, lz;   // sum w^3 r2u / ((r2u + eta2u)(rho_a + rho_b)) dv        -> laminar viscosity, Eq. 23
+#ifdef PI_ACC_F64
+  double dx = 0.0, dy = 0.0, dz = 0.0;   // the momentum sums of pair_fluid, in double (added to sx, sy, sz at the end)
+#endif
 };
 
 // One accepted ordered pair, fluid a.  DDT: include the diffusion term for this b (fluid b, or any b
@@ -69,9 +82,23 @@ __device__ __forceinline__ void pair_fluid(const DevConsts& C, float dux, float 
   A.visc = fmaxf(A.visc, mu);
   float pi = C.c_pi * fminf(dot, 0.0f) * x;      // Pi_ab, non-zero only for approaching pairs (Eq. 21)
   float coef = w3 * fmaf(P_a + vb.w, inv_rho_a * inv_rho_b, pi);
+#ifdef PI_ACC_F64
+  double coefd = (double)coef;
+#ifdef PI_TERM_F64
+  {
+    const double r2d = (double)dux * dux + (double)duy * duy + (double)duz * duz;      // du are exact (C1)
+    const double wd = fmax(1.0 - sqrt(r2d) * (C.cs / (2.0 * C.h)), 0.0);
+    coefd = wd * wd * wd * (((double)P_a + (double)vb.w) / ((double)rho_a * (double)pb.w) + (double)pi);
+  }
+#endif
+  A.dx += coefd * (double)dux;
+  A.dy += coefd * (double)duy;
+  A.dz += coefd * (double)duz;
+#else
   A.sx = fmaf(coef, dux, A.sx);
   A.sy = fmaf(coef, duy, A.sy);
   A.sz = fmaf(coef, duz, A.sz);
+#endif
   if (C.visco_model == 1) {                      // Eq. 23 (c_pi = 0 in this model)
     float lam = w3 * r2u * x;
     A.lx = fmaf(lam, dvx, A.lx);
@@ -96,9 +123,16 @@ __device__ __forceinline__ void pair_bound(const DevConsts& C, float dux, float 
 __device__ __forceinline__ float4 finish_particle(const DevConsts& C, bool fluid, float rho_a, const PairAcc& A) {
   float4 r;
   if (fluid) {
+#ifdef PI_ACC_F64
+    const double cm = -C.mass * (-5.0 * C.aD / (C.h * C.h)) * C.cs;      // c_mom before its rounding to float
+    r.x = (float)(cm * (A.dx + (double)A.sx) + (double)C.g[0]);
+    r.y = (float)(cm * (A.dy + (double)A.sy) + (double)C.g[1]);
+    r.z = (float)(cm * (A.dz + (double)A.sz) + (double)C.g[2]);
+#else
     r.x = fmaf(C.c_mom, A.sx, C.g[0]);
     r.y = fmaf(C.c_mom, A.sy, C.g[1]);
     r.z = fmaf(C.c_mom, A.sz, C.g[2]);
+#endif
     if (C.visco_model == 1) {
       r.x = fmaf(C.c_lam, A.lx, r.x);
       r.y = fmaf(C.c_lam, A.ly, r.y);
