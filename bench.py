@@ -224,6 +224,8 @@ def run_ours(args):
     n = case.n
     stream = torch.cuda.current_stream()
     prm = dict(case.params, integrator=1 if args.integrator == "verlet" else 0)
+    compensated = args.compensated if args.compensated >= 0 else (1 if args.config == 4 else 0)
+    prm["compensated_sums"] = compensated
     if args.mdbc:
         prm.update(boundary_model=1, mdbc_slip=1)
     if args.shifting:
@@ -387,6 +389,7 @@ def run_ours(args):
             "config": {"workload": case.name, "n_particles": n, "n_fluid": case.n_fluid, "n_boundary": case.n_bound,
                        "cell_div": cell_div, "pi_kernel": int(info0.pi_kernel), "integrator": args.integrator, "multi_gpu": "replicas only",
                        "boundary_model": "mdbc" if args.mdbc else "dbc", "shifting": bool(args.shifting),
+                       "compensated_sums": compensated,
                        "developed_steps": args.develop + max(args.warmup, 3),
                        "warmup_requested": args.warmup,      # fewer than 3 are raised to 3 (timing rules)
                        "timing": "value: CUDA events around K steps with the per-phase timers off; phase_ms_per_step and roofline: a second loop of K steps with the timers on",
@@ -419,6 +422,9 @@ def main():
     ap.add_argument("--pi-kernel", type=int, default=0)
     ap.add_argument("--integrator", choices=["symplectic", "verlet"], default="symplectic",
                     help="symplectic (default, the metric's configuration) or verlet (Eq. 30-31, one pass per step)")
+    ap.add_argument("--compensated", type=int, default=-1,
+                    help="sph_params.compensated_sums (Kahan momentum sums, +15 %% per pass); default 1 on config 4, where the "
+                         "stated tolerance needs it, else 0")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-legs", action="store_true",
                     help="also time legs B1 (config 0, 100 steps, 1 core) and B3 (config 3 sub-cube, one pass) of BASELINE.md "

@@ -94,6 +94,13 @@ typedef struct sph_params {
                              /*   particle and follows Eq. 54 (A29); 0 disables the free-surface form       */
   double shift_alpha_n;      /* a_n of Eq. 54 ("0 for violent flows, 0.1 for long slow flows")              */
   double shift_beta_n;       /* beta_n of Eq. 54 (initial concentration gradient)                           */
+  int32_t compensated_sums;  /* 1: the momentum sums of Eq. 22 are accumulated with a running compensation  */
+                             /*   (Kahan).  Under deep hydrostatic pressure the pair terms add up to ~100    */
+                             /*   times the net acceleration and plain fp32 sums leave a few 1e-5 m/s^2; with */
+                             /*   this option the full-size config 4 meets rel 1e-4 / floor 1e-6 max|a| for   */
+                             /*   every particle, at +15 % time per interaction pass.  Default 0.  The quad   */
+                             /*   and gather kernels have it; where the tiled kernel would run (pi_kernel 2,  */
+                             /*   2-D, cell_div > 1) the gather kernel runs instead (sph_info.pi_kernel = 1). */
   sph_alloc_fn dev_alloc;    /* may be NULL (cudaMalloc)                                             */
   sph_free_fn dev_free;      /* may be NULL (cudaFree)                                               */
   void* user;                /* passed back to dev_alloc / dev_free                                  */

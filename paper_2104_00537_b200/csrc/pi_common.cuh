@@ -52,10 +52,34 @@ struct PairAcc {
   float sd;           // sum_F (1/rho_b) w^3 (rho_a - rho_b)                  -> density diffusion, Eq. 17-18 (A3)
   float visc;         // max |mu_ab| / c_mu
   float lx, ly, lz;   // sum w^3 r2u / ((r2u + eta2u)(rho_a + rho_b)) dv        -> laminar viscosity, Eq. 23
+  float kx, ky, kz;   // running compensation of sx, sy, sz (sph_params.compensated_sums; 0 otherwise)
 #ifdef PI_ACC_F64
   double dx = 0.0, dy = 0.0, dz = 0.0;   // the momentum sums of pair_fluid, in double (added to sx, sy, sz at the end)
 #endif
 };
+
+// s += p with the Kahan compensation c (what the rounded sum has in excess of the exact one); no fast-math, so the
+// compiler keeps (t - s) - y as written.
+__device__ __forceinline__ void kahan_add(float p, float& s, float& c) {
+  const float y = p - c;
+  const float t = s + y;
+  c = (t - s) - y;
+  s = t;
+}
+
+// Momentum sums of Eq. 22: A.s += coef * du.  Plain FMA, or compensated when sph_params.compensated_sums = 1 (under deep
+// hydrostatic pressure the pair terms are ~100 times the net acceleration; profiles/r3_momentum_error_split.md).
+__device__ __forceinline__ void momentum_add(const DevConsts& C, float coef, float dux, float duy, float duz, PairAcc& A) {
+  if (C.comp_sums) {                             // uniform branch
+    kahan_add(coef * dux, A.sx, A.kx);
+    kahan_add(coef * duy, A.sy, A.ky);
+    kahan_add(coef * duz, A.sz, A.kz);
+  } else {
+    A.sx = fmaf(coef, dux, A.sx);
+    A.sy = fmaf(coef, duy, A.sy);
+    A.sz = fmaf(coef, duz, A.sz);
+  }
+}
 
 // One accepted ordered pair, fluid a.  DDT: include the diffusion term for this b (fluid b, or any b
 // when ddt_over_boundary; A4).
@@ -95,9 +119,7 @@ __device__ __forceinline__ void pair_fluid(const DevConsts& C, float dux, float 
   A.dy += coefd * (double)duy;
   A.dz += coefd * (double)duz;
 #else
-  A.sx = fmaf(coef, dux, A.sx);
-  A.sy = fmaf(coef, duy, A.sy);
-  A.sz = fmaf(coef, duz, A.sz);
+  momentum_add(C, coef, dux, duy, duz, A);
 #endif
   if (C.visco_model == 1) {                      // Eq. 23 (c_pi = 0 in this model)
     float lam = w3 * r2u * x;
@@ -129,9 +151,9 @@ __device__ __forceinline__ float4 finish_particle(const DevConsts& C, bool fluid
     r.y = (float)(cm * (A.dy + (double)A.sy) + (double)C.g[1]);
     r.z = (float)(cm * (A.dz + (double)A.sz) + (double)C.g[2]);
 #else
-    r.x = fmaf(C.c_mom, A.sx, C.g[0]);
-    r.y = fmaf(C.c_mom, A.sy, C.g[1]);
-    r.z = fmaf(C.c_mom, A.sz, C.g[2]);
+    r.x = fmaf(C.c_mom, A.sx - A.kx, C.g[0]);    // k = 0 without compensated sums
+    r.y = fmaf(C.c_mom, A.sy - A.ky, C.g[1]);
+    r.z = fmaf(C.c_mom, A.sz - A.kz, C.g[2]);
 #endif
     if (C.visco_model == 1) {
       r.x = fmaf(C.c_lam, A.lx, r.x);

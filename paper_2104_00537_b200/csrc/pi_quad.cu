@@ -139,7 +139,16 @@ struct PairAcc2 {
   float visc;         // max |mu_ab| / c_mu over the accepted pairs of both a (only the maximum over all particles is used, Eq. 35)
   f2 nb;              // neighbour counts, kept as floats (exact integers)
   f2 lx, ly, lz;      // laminar viscosity sums, Eq. 23 (LAM instantiations only)
+  f2 cx, cy, cz;      // running compensation of sx, sy, sz (KAHAN instantiations only: sph_params.compensated_sums)
 };
+// Kahan update s += a * b with the running compensation c (c = what the rounded sum has in excess of the exact one).
+__device__ __forceinline__ void f2_kahan_acc(f2 a, f2 b, f2& s, f2& c) {
+  const f2 m1 = f2_bc(-1.0f);
+  const f2 y = f2_fma(c, m1, f2_mul(a, b));        // a b - c
+  const f2 t = f2_add(s, y);
+  c = f2_fma(y, m1, f2_fma(s, m1, t));             // (t - s) - y
+  s = t;
+}
 // One popped candidate b against both a of the lane (Eq. 15, 17-18, 21-22, 36), branch free, in two parts so that
 // the record registers are free again after the head (the P loop reloads them for the next step before the tail).
 // A b outside the support of a_h (prefilter false positive, neighbour of the other a only, or the dummy record)
@@ -165,7 +174,7 @@ __device__ __forceinline__ void pair2_head(const PairA& a, const float4 pb, cons
     T.ppb = f2_mul(a.inv_rho, f2_bc(vb.w));       // kap_b / rho_a
   }
 }
-template <bool A_FLUID, bool DDT, bool LAM, bool FOURT>
+template <bool A_FLUID, bool DDT, bool LAM, bool FOURT, bool KAHAN>
 __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, const PairTmp& T, PairAcc2& A) {
   f2 r2 = f2_mul(T.dux, T.dux);                   // C2: individually rounded
   r2 = f2_fma(T.duy, T.duy, r2);
@@ -210,9 +219,15 @@ __device__ __forceinline__ void pair2_tail(const DevConsts& C, const PairA& a, c
     // (Pa + Pb) / (rho_a rho_b) = kap_a / rho_b + kap_b / rho_a
     const f2 pp = f2_fma(a.kap, f2_bc(T.inv_rho_b), T.ppb);
     const f2 coef = f2_mul(w3, f2_fma(f2_bc(C.c_pi), t, pp));
-    f2_fma_acc(coef, T.dux, A.sx);
-    f2_fma_acc(coef, T.duy, A.sy);
-    f2_fma_acc(coef, T.duz, A.sz);
+    if (KAHAN) {   // compensated momentum sums: the pair terms are ~100x the net under deep hydrostatic pressure
+      f2_kahan_acc(coef, T.dux, A.sx, A.cx);
+      f2_kahan_acc(coef, T.duy, A.sy, A.cy);
+      f2_kahan_acc(coef, T.duz, A.sz, A.cz);
+    } else {
+      f2_fma_acc(coef, T.dux, A.sx);
+      f2_fma_acc(coef, T.duy, A.sy);
+      f2_fma_acc(coef, T.duz, A.sz);
+    }
   }
 }
 
@@ -291,7 +306,7 @@ __device__ __forceinline__ void mma_m16n8k8(unsigned& d0, unsigned& d1, unsigned
 // A_FLUID ? 1 : 0, staged at [cell_start + 16*grp, ...).  bmw is this warp's word-list area ([QSLOT][32] uint2).
 // Lane (g, t) = (lane / 4, lane % 4): the 4 lanes of g own the pair (a_2g, a_2g+1); lane t owns the candidates
 // whose staged index is congruent to 2t or 2t+1 modulo 8.
-template <bool A_FLUID, bool LAM, bool FOURT>
+template <bool A_FLUID, bool LAM, bool FOURT, bool KAHAN>
 __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& A, const QSmem& S, uint2* bmw, int cx,
                                               int cy, int cz, unsigned cell_start, unsigned n_a, unsigned grp, int part,
                                               unsigned total, float& viscmax, unsigned int& nbsum) {
@@ -346,6 +361,7 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   acc.lx = acc.ly = acc.lz = f2_pack(0.f, 0.f);
   acc.sx = acc.sy = acc.sz = acc.sc = acc.sd = acc.nb = f2_pack(0.f, 0.f);
   acc.visc = 0.f;
+  acc.cx = acc.cy = acc.cz = f2_pack(0.f, 0.f);
 
   // Rounds are homogeneous in the type block of b: fluid a sweeps the 9 boundary-block rows first (diffusion
   // term only if ddt_over_boundary, A4), then the 9 fluid rows; boundary a sweeps the fluid rows only (Eq. 36).
@@ -483,17 +499,26 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   if (LAM) {                                                                                           \
     q_s[10] = f2_lo(acc.lx); q_s[11] = f2_hi(acc.lx); q_s[12] = f2_lo(acc.ly); q_s[13] = f2_hi(acc.ly); \
     q_s[14] = f2_lo(acc.lz); q_s[15] = f2_hi(acc.lz);                                                 \
+  }                                                                                                    \
+  Q_UNPACK_K()
+#define Q_UNPACK_K()                                                                                   \
+  if (KAHAN) {                                                                                         \
+    q_s[18] = f2_lo(acc.cx); q_s[19] = f2_hi(acc.cx); q_s[20] = f2_lo(acc.cy); q_s[21] = f2_hi(acc.cy); \
+    q_s[22] = f2_lo(acc.cz); q_s[23] = f2_hi(acc.cz);                                                 \
   }
+#define Q_PACK_K()                                                                                     \
+  if (KAHAN) { acc.cx = f2_pack(q_s[18], q_s[19]); acc.cy = f2_pack(q_s[20], q_s[21]); acc.cz = f2_pack(q_s[22], q_s[23]); }
 #define Q_PACK()                                                                                       \
   acc.sx = f2_pack(q_s[0], q_s[1]); acc.sy = f2_pack(q_s[2], q_s[3]); acc.sz = f2_pack(q_s[4], q_s[5]); \
   acc.sc = f2_pack(q_s[6], q_s[7]); acc.sd = f2_pack(q_s[8], q_s[9]); acc.nb = f2_pack(q_s[16], q_s[17]); \
-  if (LAM) { acc.lx = f2_pack(q_s[10], q_s[11]); acc.ly = f2_pack(q_s[12], q_s[13]); acc.lz = f2_pack(q_s[14], q_s[15]); }
+  if (LAM) { acc.lx = f2_pack(q_s[10], q_s[11]); acc.ly = f2_pack(q_s[12], q_s[13]); acc.lz = f2_pack(q_s[14], q_s[15]); } \
+  Q_PACK_K()
 #define Q_LOOP(DDT)                                                                                    \
   {                                                                                                    \
     float4 pbA, vbA, pbB, vbB;                                                                         \
     PairTmp T;                                                                                         \
     unsigned addr;                                                                                     \
-    float q_s[18];             /* the packed sums, as scalars across the back edge of the loop */      \
+    float q_s[24];             /* the packed sums, as scalars across the back edge of the loop */      \
     Q_POP(addr)                                                                                        \
     Q_LOAD(addr, pbA, vbA)                                                                             \
     Q_POP(addr)                                                                                        \
@@ -504,11 +529,11 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
       Q_LOAD(addr, pbB, vbB)   /* record of step k + 1: its address was popped during step k - 1 */    \
       Q_POP(addr)              /* address of step k + 2 */                                             \
       pair2_head<A_FLUID, DDT>(a, pbA, vbA, T);                                                        \
-      pair2_tail<A_FLUID, DDT, LAM, FOURT>(C, a, T, acc);                                              \
+      pair2_tail<A_FLUID, DDT, LAM, FOURT, KAHAN>(C, a, T, acc);                                              \
       Q_LOAD(addr, pbA, vbA)                                                                           \
       Q_POP(addr)                                                                                      \
       pair2_head<A_FLUID, DDT>(a, pbB, vbB, T);                                                        \
-      pair2_tail<A_FLUID, DDT, LAM, FOURT>(C, a, T, acc);                                              \
+      pair2_tail<A_FLUID, DDT, LAM, FOURT, KAHAN>(C, a, T, acc);                                              \
       Q_UNPACK()                                                                                       \
     }                                                                                                  \
     Q_PACK()                                                                                           \
@@ -517,6 +542,8 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
 #undef Q_LOOP
 #undef Q_PACK
 #undef Q_UNPACK
+#undef Q_PACK_K
+#undef Q_UNPACK_K
 #undef Q_LOAD
 #undef Q_CHECK_ADDR
 #undef Q_POP
@@ -527,6 +554,11 @@ __device__ __forceinline__ void process_group(const DevConsts& C, const PiArgs& 
   r0.sc = qsum(f2_lo(acc.sc)); r1.sc = qsum(f2_hi(acc.sc));
   const unsigned nb0 = (unsigned)qsum(f2_lo(acc.nb)), nb1 = (unsigned)qsum(f2_hi(acc.nb));
   if (A_FLUID) {
+    if (KAHAN) {
+      acc.sx = f2_fma(acc.cx, f2_bc(-1.0f), acc.sx);   // sum - compensation
+      acc.sy = f2_fma(acc.cy, f2_bc(-1.0f), acc.sy);
+      acc.sz = f2_fma(acc.cz, f2_bc(-1.0f), acc.sz);
+    }
     r0.sx = qsum(f2_lo(acc.sx)); r1.sx = qsum(f2_hi(acc.sx));
     r0.sy = qsum(f2_lo(acc.sy)); r1.sy = qsum(f2_hi(acc.sy));
     r0.sz = qsum(f2_lo(acc.sz)); r1.sz = qsum(f2_hi(acc.sz));
@@ -613,7 +645,7 @@ __global__ void __launch_bounds__(256) k_quad_tiles(DevConsts C, const uint32_t*
 }
 
 // Persistent kernel: one CTA per SM takes active tiles from the list until it is used up.
-template <int NT, int NMAX, bool LAM, bool FOURT>
+template <int NT, int NMAX, bool LAM, bool FOURT, bool KAHAN>
 __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int ntx, int nty) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int NWARP = NT / 32;
@@ -809,8 +841,8 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
     const int blk = 1 - (s >> 3), cz = (s >> 2) & 1, cy = (s >> 1) & 1, cx = s & 1;
     const int rr = qrange(blk, 1 + cx, 1 + cy, 1 + cz);
     const unsigned cell_start = S.soff[rr], n_a = s_cnt[rr], grp = gi - S.seg[1 + s];
-    if (blk == 1) process_group<true, LAM, FOURT>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
-    else process_group<false, false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
+    if (blk == 1) process_group<true, LAM, FOURT, KAHAN>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
+    else process_group<false, false, false, false>(C, A, S, bmw, cx, cy, cz, cell_start, n_a, grp, part, total, viscmax, nbsum);
   }
   // This thread is done with the staged records: its generic-proxy accesses (the in-place rewrite of step 3, the dummy
   // record, the reads of step 4) are ordered before the next barrier here, in the thread that made them, so that the
@@ -823,14 +855,14 @@ __global__ void __launch_bounds__(NT, 1) k_pi_quad(DevConsts C, PiArgs A, int nt
   reduce_scalars(A.sc, f2max, viscmax, nbsum);
 }
 
-template <int NT, int NMAX, bool LAM, bool FOURT>
+template <int NT, int NMAX, bool LAM, bool FOURT, bool KAHAN>
 int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   const int ntx = (C.nc[0] + QT - 1) / QT, nty = (C.nc[1] + QT - 1) / QT, ntz = (C.nc[2] + QT - 1) / QT;
   constexpr int NWARP = NT / 32;
   const size_t smem = sizeof(float4) * 2 * NMAX + sizeof(uint2) * NMAX +
                       sizeof(uint2) * NWARP * QSLOT * 32 + sizeof(uint32_t) * ((QNR + 1) + QNR + (QNSEG + 2));
   // per device, so set on every launch (a cheap host call): a process may hold contexts on several devices
-  if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM, FOURT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+  if (cudaFuncSetAttribute(k_pi_quad<NT, NMAX, LAM, FOURT, KAHAN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
       cudaSuccess) {
     cudaGetLastError();
     return -1;
@@ -844,7 +876,7 @@ int launch_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (cudaMemsetAsync(A.acc, 0, sizeof(float4) * (size_t)A.n, s) != cudaSuccess) return -1;
   if (A.nbcount && cudaMemsetAsync(A.nbcount, 0, sizeof(uint32_t) * (size_t)A.n, s) != cudaSuccess) return -1;
   k_quad_tiles<<<(unsigned)((ntiles + 255) / 256), 256, 0, s>>>(C, A.cellstart, ntx, nty, (int)ntiles, A.tile_ws);
-  k_pi_quad<NT, NMAX, LAM, FOURT><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
+  k_pi_quad<NT, NMAX, LAM, FOURT, KAHAN><<<(unsigned)min((long long)n_sm, ntiles), NT, smem, s>>>(C, A, ntx, nty);
 #ifdef Q_STATS
   k_qstats_print<<<1, 1, 0, s>>>();
 #endif
@@ -868,8 +900,14 @@ int pi_quad(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   // the packed Fourtakas term uses the series form of the inverse EOS (exact to fp32 rounding for |e| <= 0.02)
   if (C.ddt_model == 1 && !C.hyd_series_ok) return -1;
   const bool lam = C.visco_model == 1, fourt = C.ddt_model == 1;   // Eq. 23 / Eq. 19-20 instantiations
-  if (lam && fourt) return launch_quad<512, 4928, true, true>(C, A, s);
-  if (lam) return launch_quad<512, 4928, true, false>(C, A, s);
-  if (fourt) return launch_quad<512, 4928, false, true>(C, A, s);
-  return launch_quad<512, 4928, false, false>(C, A, s);
+  if (C.comp_sums) {                                               // sph_params.compensated_sums: Kahan momentum sums
+    if (lam && fourt) return launch_quad<512, 4928, true, true, true>(C, A, s);
+    if (lam) return launch_quad<512, 4928, true, false, true>(C, A, s);
+    if (fourt) return launch_quad<512, 4928, false, true, true>(C, A, s);
+    return launch_quad<512, 4928, false, false, true>(C, A, s);
+  }
+  if (lam && fourt) return launch_quad<512, 4928, true, true, false>(C, A, s);
+  if (lam) return launch_quad<512, 4928, true, false, false>(C, A, s);
+  if (fourt) return launch_quad<512, 4928, false, true, false>(C, A, s);
+  return launch_quad<512, 4928, false, false, false>(C, A, s);
 }

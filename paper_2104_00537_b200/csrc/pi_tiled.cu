@@ -114,7 +114,7 @@ __device__ __forceinline__ void pair_eval(const DevConsts& C, const LaneA& a, co
     A.visc = fmaxf(A.visc, fabsf(dot) * x * rs);       // |mu_ab| / c_mu   (Eq. 21, A12)
     const float t = fminf(dot, 0.0f) * x;              // Pi_ab = c_pi * t, approaching pairs only (Eq. 21)
     const float coef = w3 * fmaf(a.P + P.Pb, a.inv_rho * inv_rho_b, C.c_pi * t);
-    A.sx = fmaf(coef, dux, A.sx);
+    A.sx = fmaf(coef, dux, A.sx);                      // plain sums only: pi_tiled() declines compensated_sums
     A.sy = fmaf(coef, duy, A.sy);
     A.sz = fmaf(coef, duz, A.sz);
     if (C.visco_model == 1) {                          // Eq. 23 (A22; c_pi = 0 in this model); uniform branch
@@ -444,6 +444,7 @@ int launch_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
 int pi_tiled(const DevConsts& C, const PiArgs& A, cudaStream_t s) {
   if (A.n == 0) return 0;
   if (C.k != 1) return -1;
+  if (C.comp_sums) return -1;        // no compensated variant of this kernel: the caller runs the gather kernel (sph.h)
   if (!(C.eta2u > 0.f)) return -1;   // the self pair (r = 0) must evaluate to exactly 0, which needs eta^2 > 0
   if (C.dim == 3) return launch_tiled<3, 512, 4992>(C, A, s);
   return launch_tiled<2, 128, 1024>(C, A, s);

@@ -182,6 +182,7 @@ int validate(const sph_params* p, std::string& why) {
   if (p->mdbc_det_min < 0) return bad("mdbc_det_min must be >= 0");
   if (p->shift_model < 0 || p->shift_model > 1) return bad("shift_model must be 0 (none) or 1 (Fickian shifting)");
   if (p->shift_coef < 0 || p->shift_fs_conc < 0) return bad("shift_coef and shift_fs_conc must be >= 0");
+  if (p->compensated_sums < 0 || p->compensated_sums > 1) return bad("compensated_sums must be 0 or 1");
   const double cs_min = 2.0 * p->h / p->cell_div;
   if (p->cell_size != 0.0 && p->cell_size < cs_min * (1.0 - 1e-12)) return bad("cell_size smaller than 2h/cell_div");
   for (int k = 0; k < 3; k++) {
@@ -241,6 +242,7 @@ int derive(const sph_params* p, DevConsts& C, std::string& why) {
   C.c_mu = (float)(p->h / cs);
   C.ddt_over_boundary = p->ddt_over_boundary;
   C.rho_bound_floor = p->rho_bound_floor;
+  C.comp_sums = p->compensated_sums;
   C.ddt_model = p->ddt_model;
   {
     // Fourtakas DDT (Eq. 19-20, A23): rho^H_ab = rho0 [(1 + e)^(1/gamma) - 1], e = rho0 g.r_ab / B, |r_ab| < 2h

@@ -25,6 +25,7 @@ struct DevConsts {
   float c_pi;              // -alpha c0 * 2 * (h/cs) : Pi_ab  = c_pi * min(dv.du,0) / ((r2u+eta2u)(rho_a+rho_b))
   float c_mu;              // h/cs                   : mu_ab  = c_mu * (dv.du) / (r2u + eta2u)
   int ddt_over_boundary, rho_bound_floor;
+  int comp_sums;           // sph_params.compensated_sums: Kahan accumulation of the momentum sums of Eq. 22
   int visco_model;         // 0 artificial (Eq. 21-22), 1 laminar (Eq. 23)
   int ddt_model;           // 0 Molteni (Eq. 18), 1 Fourtakas (Eq. 19-20)
   int hyd_series_ok;       // |e| <= 0.02 for every pair: the binomial series below is exact to fp32 rounding

@@ -56,6 +56,7 @@ class SphParams(C.Structure):
         ("shift_fs_conc", C.c_double),
         ("shift_alpha_n", C.c_double),
         ("shift_beta_n", C.c_double),
+        ("compensated_sums", C.c_int32),
         ("dev_alloc", ALLOC_FN),
         ("dev_free", FREE_FN),
         ("user", C.c_void_p),
@@ -171,7 +172,7 @@ class Sph:
         sp.visco_model = int(params.get("visco_model", 0))
         sp.nu0 = float(params.get("nu0", 0.0))
         sp.ddt_model = int(params.get("ddt_model", 0))
-        for k in ("boundary_model", "mdbc_slip", "shift_model"):
+        for k in ("boundary_model", "mdbc_slip", "shift_model", "compensated_sums"):
             setattr(sp, k, int(params.get(k, 0)))
         for k in ("mdbc_det_min", "shift_coef", "shift_fs_conc", "shift_alpha_n", "shift_beta_n"):
             setattr(sp, k, float(params.get(k, 0.0)))
